@@ -1,0 +1,155 @@
+/*
+ * fourphonon.h -- C ABI of the B200-native FourPhonon scattering-rate library (libfourphonon_b200.so).
+ *
+ * The library evaluates the hot path of FourPhonon_GPU (arXiv 2510.00518): three-phonon (+,-) and four-phonon
+ * (++,+-,--) scattering rates of target modes lambda=(q,j) on a uniform Gamma-centred q-mesh under the RTA, plus
+ * the RTA thermal conductivity.  Every step runs in hand-written sm_100a CUDA kernels; there is no CPU fallback.
+ * Operation definitions: PAPER.md (Algorithm 1; Algorithms 3-5) with the
+ * formulas the paper defers to its references taken from SURVEY.md §8(c) steps 1-8 (readings in DESIGN.md §3).
+ *
+ * Conventions
+ *   mesh N1 x N2 x N3, N = N1*N2*N3 q-points, iq = i1 + N1*(i2 + N2*i3), q = sum_mu (i_mu/N_mu) b_mu
+ *   nb = 3*natoms branches, mode index lambda = iq*nb + j
+ *   units: omega rad/ps, v_g Angstrom/ps, lengths Angstrom, masses u, Phi3 eV/A^3, Phi4 eV/A^4, T K,
+ *          rates 1/ps, kappa W/(m K)
+ *   channels: 3ph index 0 = "+" (q'' = q + q'), 1 = "-" (q'' = q - q');
+ *             4ph index 0 = "++" (q''' = q + q' + q''), 1 = "+-" (q + q' - q''), 2 = "--" (q - q' - q'')
+ *
+ * Memory
+ *   Every array argument is documented HOST or DEVICE.  Arguments marked "loc" are host or device pointers as stated
+ *   by the accompanying fp_memloc value; with FP_MEM_HOST the library performs the copies itself on `stream` (these
+ *   are the end-to-end entry points: host<->device traffic happens inside the call).
+ *   The library never calls cudaMalloc for data: all device storage is carved out of the caller-provided `workspace`
+ *   (a DEVICE allocation, 256-byte aligned, owned by the caller, which must outlive the context).  Inputs of
+ *   fp_setup are copied/derived into the workspace; they are NOT borrowed and may be freed after fp_setup returns.
+ *
+ * Execution
+ *   All kernels and copies are issued on `stream` (a cudaStream_t passed as void*, NULL = default stream).
+ *   fp_setup, fp_rates3 and fp_rates4 synchronise the stream internally (chunk planning reads a few bytes of
+ *   device-side counts back; Algorithm 5 is the same mode-by-mode host loop), so on return the
+ *   outputs are complete.  fp_kappa_rta with FP_MEM_DEVICE outputs is asynchronous.
+ *
+ * Errors
+ *   Every call returns FP_OK (0) or a negative code; nothing throws or aborts.  fp_last_error(ctx) (ctx may be NULL
+ *   for setup failures) returns a static/ctx-owned message.
+ */
+#ifndef FOURPHONON_H
+#define FOURPHONON_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define FP_OK       0
+#define FP_EINVAL  (-1)   /* bad argument / shape / value                         */
+#define FP_ENOMEM  (-2)   /* workspace too small                                  */
+#define FP_ECUDA   (-3)   /* a CUDA runtime call or kernel failed                 */
+#define FP_ESTATE  (-4)   /* call order (e.g. fp_rates4 without IFC4 at setup)    */
+
+typedef struct fp_ctx fp_ctx;                       /* opaque, host-side handle */
+
+typedef enum { FP_MEM_HOST = 0, FP_MEM_DEVICE = 1 } fp_memloc;
+
+typedef struct {
+    double  lattvec[9];     /* rows a1,a2,a3, Cartesian, Angstrom                                                  */
+    int32_t natoms;         /* atoms per cell (positions are not needed by the rate path)                          */
+} fp_crystal;
+
+/* Anharmonic force-constant list (HOST pointers; analysed on the host at setup).
+ * Cluster t is anchored at basis atom atoms[t*ord+0] in cell 0; the other ord-1 atoms sit in cells cells[t][m][0..2]. */
+typedef struct {
+    int64_t        n;       /* number of clusters (triplets for ord=3, quartets for ord=4)                         */
+    const int32_t *atoms;   /* n*ord   basis indices (i,j,k[,l]), 0-based                                          */
+    const int32_t *cells;   /* n*(ord-1)*3 integer cell offsets of j,k[,l]                                         */
+    const double  *phi;     /* n*3^ord, index order alpha slowest ... last Cartesian index fastest                 */
+} fp_ifc;
+
+/* Adaptive Gaussian broadening (compute_sigma).                              */
+typedef struct {
+    double scale;           /* "scalebroad"; BASELINE configs use 1.0; must be > 0                                 */
+    double ncut;            /* window half-width in sigma: 2.0 = PAPER.md:163; INFINITY disables the filter        */
+    double sigma_const;     /* 0 -> adaptive sigma; > 0 -> this sigma (rad/ps) for every process (test mode,       */
+                            /* adaptive sigma is identically 0 on 2x2x2 meshes)           */
+} fp_broadening;
+
+/* Device-time profile of the kernels launched since the last fp_profile_reset (CUDA events on the launch stream).   */
+typedef struct {
+    double  ms_count, ms_scan, ms_fill, ms_precontract, ms_contract, ms_reduce;  /* summed launch durations, ms     */
+    int64_t n_count, n_scan, n_fill, n_precontract, n_contract, n_reduce;        /* launches                        */
+    int64_t candidates;     /* momentum-conserving candidates examined by the count pass                            */
+    int64_t processes;      /* allowed processes evaluated by the contraction kernels                               */
+    double  contract_flops; /* FP64 flops executed by the contraction kernels (analytic model)        */
+    int64_t chunks;         /* list chunks                                                                          */
+} fp_profile;
+
+/* Bytes of workspace fp_setup needs for its resident tables plus `scratch_bytes` of per-call scratch (row arrays +
+ * process-list buffer; larger scratch = fewer chunks).  ifc3/ifc4 may be NULL.  Returns 0 on invalid arguments.     */
+size_t fp_workspace_bytes(const fp_crystal *crystal, const int32_t mesh[3], const fp_ifc *ifc3, const fp_ifc *ifc4,
+                          size_t scratch_bytes);
+
+/* a1 of SURVEY.md §8(a): build the resident tables (B_mu = b_mu/N_mu, BE occupations f_lambda, mass-
+ * scaled eigenvectors, mode records, Bloch phase table (a4), IFC block structure).
+ *   masses   HOST natoms (u)
+ *   omega    loc  N*nb            (rad/ps; the three Gamma acoustic modes must be exactly 0.0, item 8)
+ *   eig      loc  N*nb*nb*2       [iq][j][3*atom+alpha][re,im]
+ *   vg       loc  N*nb*3          (Angstrom/ps)
+ *   ifc3, ifc4 may be NULL (then fp_rates3 / fp_rates4 return FP_ESTATE)
+ * Errors: FP_EINVAL for mesh <= 0, natoms <= 0 or > 21, NaN/negative omega, 0 < omega < 1e-6*omega_max, T <= 0,
+ * scale <= 0, ncut < 0, atom index out of range, lcm(N1,N2,N3) > 4096; FP_ENOMEM if workspace_bytes is too small.  */
+int fp_setup(const fp_crystal *crystal, const double *masses, const double *omega, const double *eig, const double *vg,
+             fp_memloc mode_arrays_loc, const fp_ifc *ifc3, const fp_ifc *ifc4, const int32_t mesh[3], double T,
+             const fp_broadening *broadening, void *workspace, size_t workspace_bytes, void *stream, fp_ctx **out);
+
+/* a2+a5+a7+a8: three-phonon rates of `ntargets` target modes (Algorithms 1/3/4).
+ *   targets  loc  ntargets mode indices lambda
+ *   gamma    loc  ntargets*2  (+,-)  1/ps:  Gamma+ = (C3/N) sum WP+ |V+|^2,  Gamma- = (C3/N)(1/2) sum WP- |V-|^2
+ *   wp       loc  ntargets*2  weighted phase space (same sums without |V|^2 and C3), nullable
+ *   counts   loc  ntargets*2  number of allowed processes in the full rectangular domain (int64), nullable
+ * Zero-frequency targets get 0 everywhere.  FP_EINVAL for a target index out of range.                              */
+int fp_rates3(fp_ctx *ctx, const int32_t *targets, int64_t ntargets, double *gamma, double *wp, int64_t *counts,
+              fp_memloc loc, void *stream);
+
+/* a3+a6+a7+a8: four-phonon rates, channels (++,+-,--), summing only q' in [qp_begin, qp_end) (0, N = the full
+ * definition).  The prefactor is always C4/N^2 so disjoint q' ranges add up to the full rate.
+ *   gamma, wp: ntargets*3;  counts: ntargets*3 int64.                                                               */
+int fp_rates4(fp_ctx *ctx, const int32_t *targets, int64_t ntargets, int32_t qp_begin, int32_t qp_end, double *gamma,
+              double *wp, int64_t *counts, fp_memloc loc, void *stream);
+
+/* a9: kappa^{ab} = C_kappa/(T^2 Omega N) sum_lambda f(f+1) omega^2 v^a v^b / Gamma_lambda, skipping zero modes and
+ * modes with Gamma <= 0.   gamma_total loc N*nb (1/ps);  kappa loc 9 (row-major 3x3, W/(m K)).                      */
+int fp_kappa_rta(fp_ctx *ctx, const double *gamma_total, double *kappa, fp_memloc loc, void *stream);
+
+/* Debug export (not timed): the allowed-process list of one target and 3ph channel as (lambda', lambda'') pairs.
+ *   pairs HOST cap*2 int32; *n receives the number of allowed processes (may exceed cap; only cap are written).
+ * Order is the enumerator's (ascending q', j', j''); compare as sets.                                               */
+int fp_list3(fp_ctx *ctx, int32_t target, int32_t channel, int32_t *pairs, int64_t cap, int64_t *n, void *stream);
+
+/* Debug export: the 4ph allowed-process list of one target, channel and q' as (lambda', lambda'', lambda''') triples.
+ *   triples HOST cap*3 int32.                                                                                        */
+int fp_list4(fp_ctx *ctx, int32_t target, int32_t channel, int32_t qp, int32_t *triples, int64_t cap, int64_t *n,
+             void *stream);
+
+/* Profiling of the library's own kernels (off by default; adds two cudaEventRecord per launch).                     */
+int fp_profile_enable(fp_ctx *ctx, int on);
+int fp_profile_reset(fp_ctx *ctx);
+int fp_profile_get(fp_ctx *ctx, fp_profile *out);           /* synchronises the recorded events                      */
+
+/* Pure-DFMA microbenchmark on all SMs: measured FP64 throughput of this device in TFLOP/s (roofline denominator
+ * cross-check).                                                                                       */
+int fp_probe_fp64_tflops(void *stream, double *tflops);
+
+/* Unit constants as derived inside the library from CODATA 2018: out[0]=C3, out[1]=C4 (1/ps), out[2]=C_kappa,
+ * out[3]=hbar/kB (ps K).                                                                                              */
+void fp_constants(double out[4]);
+
+const char *fp_last_error(const fp_ctx *ctx);
+const char *fp_version(void);
+int fp_destroy(fp_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FOURPHONON_H */

@@ -1,0 +1,603 @@
+// fp_host.cu -- host side of the C ABI (include/fourphonon.h): argument checking, IFC block analysis, workspace
+// carving, chunk planning (Algorithm 5's mode-by-mode loop, generalised to list chunks) and launches.
+// All arithmetic of the method runs in the kernels of fp_kernels.cu; the only floating-point work here is the 3x3
+// reciprocal-lattice setup B_mu = b_mu/N_mu in the pinned order of SURVEY.md §8(c) step 3 and the unit constants.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <tuple>
+
+#include "fp_internal.cuh"
+
+namespace {
+
+// ---- unit constants (SURVEY.md §8(c) "Constants"), derived from CODATA 2018 ------------------------------------------
+constexpr double kHbar = 1.054571817e-34;     // J s
+constexpr double kKb = 1.380649e-23;          // J/K
+constexpr double kQe = 1.602176634e-19;       // C
+constexpr double kAmu = 1.66053906660e-27;    // kg
+const double kPi = 3.141592653589793238462643383279502884;
+
+double hbar_over_kb() { return kHbar / kKb * 1e12; }                                  // ps K
+double const_c3() {                                                                    // (pi hbar/4)(eV/A^3)^2/u^3/(rad/ps)^4 in 1/ps
+    double f = kQe * 1e30;
+    return kPi * kHbar * 0.25 * f * f / (kAmu * kAmu * kAmu) * 1e-60;
+}
+double const_c4() {                                                                    // (pi hbar^2/8)(eV/A^4)^2/u^4/(rad/ps)^5 in 1/ps
+    double f = kQe * 1e40;
+    return kPi * kHbar * kHbar * 0.125 * f * f / (kAmu * kAmu * kAmu * kAmu) * 1e-72;
+}
+double const_ckappa() { return kHbar * kHbar / kKb * 1e46; }                           // W/(m K) per unit
+
+thread_local std::string g_setup_err;
+
+int fail(fp_ctx *ctx, int code, const std::string &msg) {
+    if (ctx) ctx->err = msg; else g_setup_err = msg;
+    return code;
+}
+#define CU(call)                                                                                         \
+    do {                                                                                                 \
+        cudaError_t e_ = (call);                                                                         \
+        if (e_ != cudaSuccess)                                                                           \
+            return fail(ctx, FP_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_));              \
+    } while (0)
+
+size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+struct Bump {
+    char *base; size_t off, end;
+    template <typename T> T *take(size_t n) {
+        size_t o = align_up(off);
+        size_t b = n * sizeof(T);
+        if (o + b > end) return nullptr;
+        off = o + b;
+        return reinterpret_cast<T *>(base + o);
+    }
+    size_t left() const { size_t o = align_up(off); return o < end ? end - o : 0; }
+};
+
+int imod(long a, int n) { long r = a % n; return (int)(r < 0 ? r + n : r); }
+long gcdl(long a, long b) { while (b) { long t = a % b; a = b; b = t; } return a; }
+
+// Host-side analysis of an IFC list: group clusters into contraction blocks (atomA, atomB, dR) -- DESIGN.md §5.
+struct IfcHost {
+    int n = 0, nblk = 0, ncomp = 0;
+    std::vector<int4> meta0, meta1, blk_meta;
+    std::vector<double> phi;
+    std::vector<int> blk_start, seg;
+};
+
+int analyse_ifc(const fp_ifc *f, int order, int nat, const int32_t mesh[3], IfcHost &h, std::string &err) {
+    const int ncomp = order == 3 ? 27 : 81;
+    h.n = (int)f->n; h.ncomp = ncomp;
+    if (f->n < 0 || f->n > (1 << 24)) { err = "IFC list size out of range"; return FP_EINVAL; }
+    if (f->n > 0 && (!f->atoms || !f->cells || !f->phi)) { err = "IFC list has null arrays"; return FP_EINVAL; }
+    typedef std::tuple<int, int, int, int, int> Key;       // atomA, atomB, d1, d2, d3
+    std::map<Key, int> blocks;
+    std::vector<Key> key(h.n);
+    for (int c = 0; c < h.n; c++) {
+        const int32_t *at = f->atoms + (size_t)c * order;
+        for (int m = 0; m < order; m++)
+            if (at[m] < 0 || at[m] >= nat) { err = "IFC atom index out of range"; return FP_EINVAL; }
+        const int32_t *RA = f->cells + (size_t)c * (order - 1) * 3 + (order - 3) * 3;   // leg A: j (3ph) / k (4ph)
+        const int32_t *RB = RA + 3;                                                      // leg B: k (3ph) / l (4ph)
+        key[c] = Key(at[order - 2], at[order - 1], imod((long)RA[0] - RB[0], mesh[0]), imod((long)RA[1] - RB[1], mesh[1]),
+                     imod((long)RA[2] - RB[2], mesh[2]));
+        blocks.emplace(key[c], 0);
+    }
+    h.nblk = (int)blocks.size();
+    int id = 0;
+    h.blk_meta.resize(h.nblk);
+    h.seg.assign(nat * nat + 1, 0);
+    for (auto &kv : blocks) {                                // std::map iterates sorted by (atomA, atomB, dR)
+        kv.second = id;
+        const Key &k = kv.first;
+        h.blk_meta[id] = make_int4(std::get<0>(k) | (std::get<1>(k) << 16), std::get<2>(k), std::get<3>(k), std::get<4>(k));
+        h.seg[std::get<0>(k) * nat + std::get<1>(k) + 1]++;
+        id++;
+    }
+    for (int i = 0; i < nat * nat; i++) h.seg[i + 1] += h.seg[i];
+    std::vector<int> order_idx(h.n);
+    for (int c = 0; c < h.n; c++) order_idx[c] = c;
+    std::stable_sort(order_idx.begin(), order_idx.end(), [&](int a, int b) { return blocks[key[a]] < blocks[key[b]]; });
+    h.blk_start.assign(h.nblk + 1, 0);
+    h.meta0.resize(h.n); h.meta1.resize(h.n); h.phi.resize((size_t)h.n * ncomp);
+    for (int s = 0; s < h.n; s++) {
+        int c = order_idx[s];
+        const int32_t *at = f->atoms + (size_t)c * order;
+        const int32_t *cl = f->cells + (size_t)c * (order - 1) * 3;
+        const int32_t *RL = cl + (order - 2) * 3;            // last leg: k (3ph) / l (4ph)
+        h.blk_start[blocks[key[c]] + 1]++;
+        h.meta0[s] = make_int4(at[0], imod(RL[0], mesh[0]), imod(RL[1], mesh[1]), imod(RL[2], mesh[2]));
+        if (order == 4)                                      // level 1: atom j and Rj - Rl
+            h.meta1[s] = make_int4(at[1], imod((long)cl[0] - RL[0], mesh[0]), imod((long)cl[1] - RL[1], mesh[1]),
+                                   imod((long)cl[2] - RL[2], mesh[2]));
+        else
+            h.meta1[s] = make_int4(0, 0, 0, 0);
+        std::memcpy(&h.phi[(size_t)s * ncomp], f->phi + (size_t)c * ncomp, sizeof(double) * ncomp);
+    }
+    for (int b = 0; b < h.nblk; b++) h.blk_start[b + 1] += h.blk_start[b];
+    return FP_OK;
+}
+
+size_t ifc_resident_bytes(int64_t n, int order, int nat) {
+    size_t ncomp = order == 3 ? 27 : 81;
+    size_t b = 0;
+    b += align_up(n * sizeof(int4)) * 2 + align_up(n * ncomp * sizeof(double));
+    b += align_up((n + 1) * sizeof(int)) + align_up(n * sizeof(int4)) + align_up((nat * nat + 1) * sizeof(int));
+    return b + 256 * 8;
+}
+
+size_t tables_resident_bytes(int nat, const int32_t mesh[3], long L) {
+    size_t N = (size_t)mesh[0] * mesh[1] * mesh[2], nb = 3 * (size_t)nat, M = N * nb;
+    return align_up(M * sizeof(ModeRec)) + align_up(M * 8) + align_up(M * nb * 16) + align_up((size_t)L * 16) +
+           align_up(N * 4) + align_up(nat * 8) + 256 * 8;
+}
+
+long mesh_lcm(const int32_t mesh[3]) {
+    long L = mesh[0];
+    L = L / gcdl(L, mesh[1]) * mesh[1];
+    L = L / gcdl(L, mesh[2]) * mesh[2];
+    return L;
+}
+
+int upload_ifc(fp_ctx *ctx, Bump &bump, const IfcHost &h, IfcDev &dv, cudaStream_t st) {
+    int nat = ctx->d.nat;
+    int4 *m0 = bump.take<int4>(std::max(h.n, 1));
+    int4 *m1 = bump.take<int4>(std::max(h.n, 1));
+    double *phi = bump.take<double>(std::max<size_t>((size_t)h.n * h.ncomp, 1));
+    int *bs = bump.take<int>(h.nblk + 1);
+    int4 *bm = bump.take<int4>(std::max(h.nblk, 1));
+    int *seg = bump.take<int>(nat * nat + 1);
+    if (!m0 || !m1 || !phi || !bs || !bm || !seg) return fail(ctx, FP_ENOMEM, "workspace too small for IFC tables");
+    if (h.n > 0) {
+        CU(cudaMemcpyAsync(m0, h.meta0.data(), h.n * sizeof(int4), cudaMemcpyHostToDevice, st));
+        CU(cudaMemcpyAsync(m1, h.meta1.data(), h.n * sizeof(int4), cudaMemcpyHostToDevice, st));
+        CU(cudaMemcpyAsync(phi, h.phi.data(), h.phi.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+        CU(cudaMemcpyAsync(bm, h.blk_meta.data(), h.nblk * sizeof(int4), cudaMemcpyHostToDevice, st));
+    }
+    CU(cudaMemcpyAsync(bs, h.blk_start.data(), (h.nblk + 1) * sizeof(int), cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(seg, h.seg.data(), (nat * nat + 1) * sizeof(int), cudaMemcpyHostToDevice, st));
+    CU(cudaStreamSynchronize(st));                                   // host vectors go out of scope after setup
+    dv.n = h.n; dv.nblk = h.nblk; dv.ncomp = h.ncomp;
+    dv.cl_meta0 = m0; dv.cl_meta1 = m1; dv.phi = phi; dv.blk_start = bs; dv.blk_meta = bm; dv.seg = seg;
+    return FP_OK;
+}
+
+// ---- profiling ----------------------------------------------------------------------------------------------------------
+struct ProfScope {
+    fp_ctx *ctx; cudaStream_t st; int idx = -1;
+    ProfScope(fp_ctx *c, int cat, cudaStream_t s) : ctx(c), st(s) {
+        if (!ctx->profiling) return;
+        EventRec r; r.cat = cat;
+        if (cudaEventCreate(&r.a) != cudaSuccess || cudaEventCreate(&r.b) != cudaSuccess) return;
+        cudaEventRecord(r.a, st);
+        ctx->events.push_back(r);
+        idx = (int)ctx->events.size() - 1;
+    }
+    ~ProfScope() { if (idx >= 0) cudaEventRecord(ctx->events[idx].b, st); }
+};
+
+}  // namespace
+
+// =========================================================================================================================
+// public ABI
+// =========================================================================================================================
+extern "C" {
+
+const char *fp_version(void) { return "fourphonon-b200 0.1 (sm_100a)"; }
+
+void fp_constants(double out[4]) { out[0] = const_c3(); out[1] = const_c4(); out[2] = const_ckappa(); out[3] = hbar_over_kb(); }
+
+const char *fp_last_error(const fp_ctx *ctx) { return ctx ? ctx->err.c_str() : g_setup_err.c_str(); }
+
+size_t fp_workspace_bytes(const fp_crystal *crystal, const int32_t mesh[3], const fp_ifc *ifc3, const fp_ifc *ifc4,
+                          size_t scratch_bytes) {
+    if (!crystal || !mesh || crystal->natoms <= 0 || mesh[0] <= 0 || mesh[1] <= 0 || mesh[2] <= 0) return 0;
+    size_t b = tables_resident_bytes(crystal->natoms, mesh, mesh_lcm(mesh));
+    if (ifc3) b += ifc_resident_bytes(ifc3->n, 3, crystal->natoms);
+    if (ifc4) b += ifc_resident_bytes(ifc4->n, 4, crystal->natoms);
+    // staging of the raw mode arrays during fp_setup lives in the scratch region
+    size_t N = (size_t)mesh[0] * mesh[1] * mesh[2], nb = 3 * (size_t)crystal->natoms;
+    size_t staging = align_up(N * nb * 8) + align_up(N * nb * nb * 16) + align_up(N * nb * 24) + 1024;
+    return b + std::max(scratch_bytes, staging) + 4096;
+}
+
+int fp_setup(const fp_crystal *crystal, const double *masses, const double *omega, const double *eig, const double *vg,
+             fp_memloc loc, const fp_ifc *ifc3, const fp_ifc *ifc4, const int32_t mesh[3], double T,
+             const fp_broadening *br, void *workspace, size_t workspace_bytes, void *stream, fp_ctx **out) {
+    fp_ctx *ctx = nullptr;                                            // errors before allocation go to g_setup_err
+    if (!out) return fail(ctx, FP_EINVAL, "out is null");
+    *out = nullptr;
+    if (!crystal || !masses || !omega || !eig || !vg || !mesh || !br || !workspace)
+        return fail(ctx, FP_EINVAL, "null argument");
+    const int nat = crystal->natoms;
+    if (nat <= 0 || 3 * nat > FP_MAX_NB) return fail(ctx, FP_EINVAL, "natoms must be in [1,21]");
+    for (int m = 0; m < 3; m++)
+        if (mesh[m] <= 0 || mesh[m] > 1024) return fail(ctx, FP_EINVAL, "mesh dimensions must be in [1,1024]");
+    if (!(T > 0.0)) return fail(ctx, FP_EINVAL, "T must be > 0");
+    if (!(br->scale > 0.0)) return fail(ctx, FP_EINVAL, "broadening scale must be > 0");
+    if (!(br->ncut >= 0.0)) return fail(ctx, FP_EINVAL, "ncut must be >= 0");
+    if (!(br->sigma_const >= 0.0)) return fail(ctx, FP_EINVAL, "sigma_const must be >= 0");
+    for (int a = 0; a < nat; a++)
+        if (!(masses[a] > 0.0)) return fail(ctx, FP_EINVAL, "masses must be > 0");
+    const long L = mesh_lcm(mesh);
+    if (L > FP_MAX_L) return fail(ctx, FP_EINVAL, "lcm of the mesh dimensions exceeds 4096");
+    const size_t N = (size_t)mesh[0] * mesh[1] * mesh[2], nb = 3 * (size_t)nat, M = N * nb;
+    if (M * nb > (size_t)1 << 31 || N * nb * nb > (size_t)0xffffffffu)
+        return fail(ctx, FP_EINVAL, "mesh * branches too large for 32-bit candidate codes");
+    if ((reinterpret_cast<uintptr_t>(workspace) & 255) != 0) return fail(ctx, FP_EINVAL, "workspace must be 256-byte aligned");
+
+    IfcHost h3, h4;
+    std::string err;
+    if (ifc3) { int rc = analyse_ifc(ifc3, 3, nat, mesh, h3, err); if (rc) return fail(ctx, rc, err); }
+    if (ifc4) { int rc = analyse_ifc(ifc4, 4, nat, mesh, h4, err); if (rc) return fail(ctx, rc, err); }
+
+    ctx = new fp_ctx();
+    cudaStream_t st = (cudaStream_t)stream;
+    auto bail = [&](int code) { g_setup_err = ctx->err; if (ctx->pinned) cudaFreeHost(ctx->pinned); delete ctx; return code; };
+#undef CU
+#define CU(call)                                                                                         \
+    do {                                                                                                 \
+        cudaError_t e_ = (call);                                                                         \
+        if (e_ != cudaSuccess) {                                                                         \
+            fail(ctx, FP_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_));                     \
+            return bail(FP_ECUDA);                                                                       \
+        }                                                                                                \
+    } while (0)
+
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, dev));
+    ctx->ws = (char *)workspace; ctx->ws_bytes = workspace_bytes;
+    ctx->pinned_bytes = 1 << 20;
+    CU(cudaMallocHost(&ctx->pinned, ctx->pinned_bytes));
+
+    FpDev &d = ctx->d;
+    d.nat = nat; d.nb = (int)nb; d.N = (int)N; d.N1 = mesh[0]; d.N2 = mesh[1]; d.N3 = mesh[2];
+    d.L = (int)L; d.m1 = (int)(L / mesh[0]); d.m2 = (int)(L / mesh[1]); d.m3 = (int)(L / mesh[2]);
+    d.Lmask = (L & (L - 1)) == 0 ? (int)(L - 1) : -1;
+    d.scale = br->scale; d.ncut = br->ncut; d.sigma_const = br->sigma_const; d.T = T;
+    {   // B_mu = b_mu/N_mu, pinned order; host code is compiled with -ffp-contract=off
+        const double *a1 = crystal->lattvec, *a2 = a1 + 3, *a3 = a1 + 6;
+        double c1[3], c2[3], c3[3];
+        c1[0] = (a2[1] * a3[2]) - (a2[2] * a3[1]); c1[1] = (a2[2] * a3[0]) - (a2[0] * a3[2]); c1[2] = (a2[0] * a3[1]) - (a2[1] * a3[0]);
+        c2[0] = (a3[1] * a1[2]) - (a3[2] * a1[1]); c2[1] = (a3[2] * a1[0]) - (a3[0] * a1[2]); c2[2] = (a3[0] * a1[1]) - (a3[1] * a1[0]);
+        c3[0] = (a1[1] * a2[2]) - (a1[2] * a2[1]); c3[1] = (a1[2] * a2[0]) - (a1[0] * a2[2]); c3[2] = (a1[0] * a2[1]) - (a1[1] * a2[0]);
+        volatile double vol = (a1[0] * c1[0] + a1[1] * c1[1]) + a1[2] * c1[2];
+        if (!(std::fabs(vol) > 0.0)) { fail(ctx, FP_EINVAL, "lattice vectors are singular"); return bail(FP_EINVAL); }
+        const double twopi = 2.0 * 3.14159265358979323846;
+        for (int x = 0; x < 3; x++) {
+            d.B[0 + x] = ((twopi * c1[x]) / vol) / (double)mesh[0];
+            d.B[3 + x] = ((twopi * c2[x]) / vol) / (double)mesh[1];
+            d.B[6 + x] = ((twopi * c3[x]) / vol) / (double)mesh[2];
+        }
+        ctx->vol = std::fabs(vol);
+    }
+
+    // ---- carve resident tables -----------------------------------------------------------------------------------
+    Bump bump{ctx->ws, 0, workspace_bytes};
+    ModeRec *rec = bump.take<ModeRec>(M);
+    double *occ = bump.take<double>(M);
+    double2 *evec = bump.take<double2>(M * nb);
+    double2 *ph1d = bump.take<double2>(L);
+    int *qc = bump.take<int>(N);
+    double *masses_dev = bump.take<double>(nat);
+    if (!rec || !occ || !evec || !ph1d || !qc || !masses_dev) {
+        fail(ctx, FP_ENOMEM, "workspace too small for the mode tables"); return bail(FP_ENOMEM);
+    }
+    d.rec = rec; d.occ = occ; d.evec = evec; d.ph1d = ph1d; d.qc = qc;
+    if (ifc3) { int rc = upload_ifc(ctx, bump, h3, ctx->i3, st); if (rc) return bail(rc); ctx->has3 = true; }
+    if (ifc4) { int rc = upload_ifc(ctx, bump, h4, ctx->i4, st); if (rc) return bail(rc); ctx->has4 = true; }
+    ctx->resident = align_up(bump.off);
+
+    // ---- stage raw mode arrays (scratch region) and validate omega on the host ---------------------------------------
+    const double *d_omega = omega, *d_eig = eig, *d_vg = vg;
+    std::vector<double> h_omega(M);
+    if (loc == FP_MEM_HOST) {
+        Bump sc{ctx->ws, ctx->resident, workspace_bytes};
+        double *so = sc.take<double>(M), *se = sc.take<double>(M * nb * 2), *sv = sc.take<double>(M * 3);
+        if (!so || !se || !sv) { fail(ctx, FP_ENOMEM, "workspace too small to stage the mode arrays"); return bail(FP_ENOMEM); }
+        CU(cudaMemcpyAsync(so, omega, M * 8, cudaMemcpyHostToDevice, st));
+        CU(cudaMemcpyAsync(se, eig, M * nb * 16, cudaMemcpyHostToDevice, st));
+        CU(cudaMemcpyAsync(sv, vg, M * 24, cudaMemcpyHostToDevice, st));
+        d_omega = so; d_eig = se; d_vg = sv;
+        std::memcpy(h_omega.data(), omega, M * 8);
+    } else {
+        CU(cudaMemcpyAsync(h_omega.data(), omega, M * 8, cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+    }
+    double wmax = 0.0;
+    for (size_t m = 0; m < M; m++) {
+        double w = h_omega[m];
+        if (!(w >= 0.0) || !std::isfinite(w)) { fail(ctx, FP_EINVAL, "omega has a NaN, infinite or negative entry"); return bail(FP_EINVAL); }
+        wmax = std::max(wmax, w);
+    }
+    for (size_t m = 0; m < M; m++)
+        if (h_omega[m] > 0.0 && h_omega[m] < 1e-6 * wmax) {
+            fail(ctx, FP_EINVAL, "omega has a near-zero entry (0 < omega < 1e-6*omega_max); zero modes must be exactly 0");
+            return bail(FP_EINVAL);
+        }
+    CU(cudaMemcpyAsync(masses_dev, masses, nat * 8, cudaMemcpyHostToDevice, st));
+    launch_tables(d, d_omega, d_eig, d_vg, masses_dev, hbar_over_kb(), rec, occ, evec, ph1d, qc, st);
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(st));
+    *out = ctx;
+    return FP_OK;
+#undef CU
+#define CU(call)                                                                                         \
+    do {                                                                                                 \
+        cudaError_t e_ = (call);                                                                         \
+        if (e_ != cudaSuccess)                                                                           \
+            return fail(ctx, FP_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_));              \
+    } while (0)
+}
+
+int fp_destroy(fp_ctx *ctx) {
+    if (!ctx) return FP_OK;
+    for (auto &e : ctx->events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+    if (ctx->pinned) cudaFreeHost(ctx->pinned);
+    delete ctx;
+    return FP_OK;
+}
+
+// ---- shared driver of fp_rates3 / fp_rates4 ------------------------------------------------------------------------------
+static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t nt, int32_t qp_begin, int32_t qp_end,
+                        double *gamma, double *wp, int64_t *counts, fp_memloc loc, cudaStream_t st) {
+    if (!ctx) return FP_EINVAL;
+    const FpDev &d = ctx->d;
+    const IfcDev &f = order == 3 ? ctx->i3 : ctx->i4;
+    if (!(order == 3 ? ctx->has3 : ctx->has4)) return fail(ctx, FP_ESTATE, "no IFC list of this order was given to fp_setup");
+    if (nt < 0 || (nt > 0 && (!targets || !gamma))) return fail(ctx, FP_EINVAL, "null targets/gamma");
+    if (order == 4 && (qp_begin < 0 || qp_end > d.N || qp_begin > qp_end)) return fail(ctx, FP_EINVAL, "bad q' range");
+    if (nt == 0) return FP_OK;
+    const int nch = order == 3 ? 2 : 3;
+    const int64_t nqp = order == 3 ? 1 : (qp_end - qp_begin);
+    const int64_t rows_per_unit = order == 3 ? 1 : nqp * d.nb;      // rows per (target, channel)
+    const int64_t rows_per_target = nch * rows_per_unit;
+    const int64_t nmodes = (int64_t)d.N * d.nb;
+    const int64_t row_cands = (int64_t)d.N * d.nb * d.nb;
+
+    // host copy of the targets for validation
+    std::vector<int32_t> ht(nt);
+    if (loc == FP_MEM_HOST) std::memcpy(ht.data(), targets, nt * sizeof(int32_t));
+    else { CU(cudaMemcpyAsync(ht.data(), targets, nt * sizeof(int32_t), cudaMemcpyDeviceToHost, st)); CU(cudaStreamSynchronize(st)); }
+    for (int64_t i = 0; i < nt; i++)
+        if (ht[i] < 0 || ht[i] >= nmodes) return fail(ctx, FP_EINVAL, "target mode index out of range");
+
+    if (nqp == 0) {                                                   // empty q' range: all outputs zero
+        std::vector<double> z(nt * nch, 0.0); std::vector<int64_t> zc(nt * nch, 0);
+        cudaMemcpyKind k = loc == FP_MEM_HOST ? cudaMemcpyHostToHost : cudaMemcpyHostToDevice;
+        CU(cudaMemcpyAsync(gamma, z.data(), z.size() * 8, k, st));
+        if (wp) CU(cudaMemcpyAsync(wp, z.data(), z.size() * 8, k, st));
+        if (counts) CU(cudaMemcpyAsync(counts, zc.data(), zc.size() * 8, k, st));
+        CU(cudaStreamSynchronize(st));
+        return FP_OK;
+    }
+
+    // ---- scratch budget: per-target arrays for a super-chunk of targets + one list buffer -----------------------------
+    const size_t scratch = ctx->ws_bytes - ctx->resident;
+    const size_t pre_per_target = (order == 3 ? (size_t)f.nblk * 9 : (size_t)f.n * 27) * sizeof(double2);
+    const size_t per_target = pre_per_target + (size_t)rows_per_target * (4 + 8 + 16) + (size_t)nch * 24 + 4 + 64;
+    const size_t fixed = 64 * 1024 + (size_t)(rows_per_target / 1024 + 16) * 8;
+    const size_t list_min = (size_t)row_cands * 4;
+    if (scratch < fixed + list_min + per_target + 8192) return fail(ctx, FP_ENOMEM, "workspace scratch too small for one target");
+    int64_t nts_max = (int64_t)std::min<size_t>((size_t)nt, std::max<size_t>(1, (scratch / 2) / per_target));
+    while (nts_max > 1 && fixed + list_min + (size_t)nts_max * per_target + 65536 > scratch) nts_max /= 2;
+    while (nts_max * rows_per_target > (int64_t)1 << 30) nts_max = std::max<int64_t>(1, nts_max / 2);
+
+    const double c_over_n = order == 3 ? const_c3() / (double)d.N : const_c4() / ((double)d.N * (double)d.N);
+    const int max_chunks = 4096;
+
+    for (int64_t t0 = 0; t0 < nt; t0 += nts_max) {
+        const int64_t nts = std::min(nts_max, nt - t0);
+        const int64_t nrows = nts * rows_per_target;
+        Bump sc{ctx->ws, ctx->resident, ctx->ws_bytes};
+        int32_t *d_targets = nullptr;
+        if (loc == FP_MEM_DEVICE) d_targets = const_cast<int32_t *>(targets) + t0;
+        else {
+            d_targets = sc.take<int32_t>(nts);
+            if (!d_targets) return fail(ctx, FP_ENOMEM, "scratch");
+            CU(cudaMemcpyAsync(d_targets, targets + t0, nts * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+        }
+        double2 *pre = sc.take<double2>(nts * (pre_per_target / sizeof(double2)));
+        uint32_t *cnt = sc.take<uint32_t>(nrows);
+        int64_t *offs = sc.take<int64_t>(nrows + 1);
+        int64_t *bsums = sc.take<int64_t>(nrows / 4096 + 8);
+        double2 *partial = sc.take<double2>(nrows);
+        int64_t *plan = sc.take<int64_t>(max_chunks + 1);
+        double *o_gamma = nullptr, *o_wp = nullptr; int64_t *o_cnt = nullptr;
+        if (loc == FP_MEM_HOST || !wp || !counts) {
+            o_gamma = sc.take<double>(nts * nch); o_wp = sc.take<double>(nts * nch); o_cnt = sc.take<int64_t>(nts * nch);
+            if (!o_gamma || !o_wp || !o_cnt) return fail(ctx, FP_ENOMEM, "scratch");
+        }
+        if (!pre || !cnt || !offs || !bsums || !partial || !plan) return fail(ctx, FP_ENOMEM, "scratch");
+        const int64_t cap = (int64_t)(sc.left() / 4) - 64;
+        if (cap < row_cands) return fail(ctx, FP_ENOMEM, "workspace scratch too small for the process list");
+        uint32_t *list = sc.take<uint32_t>(cap);
+
+        RowArgs ra; ra.targets = d_targets; ra.row0 = 0; ra.qp_begin = qp_begin; ra.nqp = (int)nqp;
+        { ProfScope p(ctx, CAT_PRE, st);
+          if (order == 3) launch_pre3(d, f, d_targets, nts, pre, st); else launch_pre4(d, f, d_targets, nts, pre, st); }
+        CU(cudaGetLastError());
+        { ProfScope p(ctx, CAT_COUNT, st); launch_count(order, d, ra, nrows, cnt, st); }
+        CU(cudaGetLastError());
+        { ProfScope p(ctx, CAT_SCAN, st); launch_scan(cnt, nrows, offs, bsums, st); launch_plan(offs, nrows, cap, plan, max_chunks, st); }
+        CU(cudaGetLastError());
+        int64_t *hplan = (int64_t *)ctx->pinned;
+        CU(cudaMemcpyAsync(hplan, plan, (max_chunks + 1) * sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+        CU(cudaMemcpyAsync(hplan + max_chunks + 1, offs + nrows, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        CU(cudaGetLastError());
+        if (hplan[0] < 0) return fail(ctx, FP_ENOMEM, hplan[0] == -2 ? "one row exceeds the list capacity" : "too many list chunks");
+        const int nchunks = (int)hplan[0];
+        std::vector<int64_t> bounds(hplan + 1, hplan + 1 + nchunks);
+        const int64_t total = hplan[max_chunks + 1];
+        // row offsets needed on the host only at chunk boundaries: read them back in one small copy per chunk
+        int64_t r0 = 0;
+        for (int c = 0; c < nchunks; c++) {
+            const int64_t r1 = bounds[c];
+            int64_t base = 0;
+            CU(cudaMemcpyAsync(hplan, offs + r0, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+            CU(cudaStreamSynchronize(st));
+            base = hplan[0];
+            RowArgs rc = ra; rc.row0 = r0;
+            { ProfScope p(ctx, CAT_FILL, st); launch_fill(order, d, rc, r1 - r0, offs + r0, base, list, st); }
+            CU(cudaGetLastError());
+            { ProfScope p(ctx, CAT_CONTRACT, st);
+              launch_contract(order, d, f, rc, r1 - r0, offs + r0, base, list, pre, partial + r0, st); }
+            CU(cudaGetLastError());
+            r0 = r1;
+        }
+        CU(cudaGetLastError());
+        double *g_out = loc == FP_MEM_DEVICE ? gamma + t0 * nch : o_gamma;
+        double *w_out = (loc == FP_MEM_DEVICE && wp) ? wp + t0 * nch : o_wp;
+        int64_t *c_out = (loc == FP_MEM_DEVICE && counts) ? counts + t0 * nch : o_cnt;
+        { ProfScope p(ctx, CAT_REDUCE, st);
+          launch_finalize(order, d, d_targets, nts, rows_per_unit, partial, cnt, c_over_n, g_out, w_out, c_out, st); }
+        CU(cudaGetLastError());
+        if (loc == FP_MEM_HOST) {
+            CU(cudaMemcpyAsync(gamma + t0 * nch, g_out, nts * nch * 8, cudaMemcpyDeviceToHost, st));
+            if (wp) CU(cudaMemcpyAsync(wp + t0 * nch, w_out, nts * nch * 8, cudaMemcpyDeviceToHost, st));
+            if (counts) CU(cudaMemcpyAsync(counts + t0 * nch, c_out, nts * nch * 8, cudaMemcpyDeviceToHost, st));
+        }
+        CU(cudaStreamSynchronize(st));
+        // bookkeeping for the profile (analytic models)
+        ctx->prof.chunks += nchunks;
+        ctx->prof.processes += total;
+        ctx->prof.candidates += nrows * row_cands;
+        ctx->prof.contract_flops += (double)total * (double)f.nblk * 13.0 * 8.0;
+    }
+    return FP_OK;
+}
+
+int fp_rates3(fp_ctx *ctx, const int32_t *targets, int64_t ntargets, double *gamma, double *wp, int64_t *counts,
+              fp_memloc loc, void *stream) {
+    return rates_driver(ctx, 3, targets, ntargets, 0, 1, gamma, wp, counts, loc, (cudaStream_t)stream);
+}
+
+int fp_rates4(fp_ctx *ctx, const int32_t *targets, int64_t ntargets, int32_t qp_begin, int32_t qp_end, double *gamma,
+              double *wp, int64_t *counts, fp_memloc loc, void *stream) {
+    return rates_driver(ctx, 4, targets, ntargets, qp_begin, qp_end, gamma, wp, counts, loc, (cudaStream_t)stream);
+}
+
+int fp_kappa_rta(fp_ctx *ctx, const double *gamma_total, double *kappa, fp_memloc loc, void *stream) {
+    if (!ctx || !gamma_total || !kappa) return ctx ? fail(ctx, FP_EINVAL, "null argument") : FP_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const FpDev &d = ctx->d;
+    const size_t M = (size_t)d.N * d.nb;
+    const double pref = const_ckappa() / (d.T * d.T * ctx->vol * (double)d.N);
+    if (loc == FP_MEM_DEVICE) {
+        launch_kappa(d, gamma_total, pref, kappa, st);
+        CU(cudaGetLastError());
+        return FP_OK;
+    }
+    Bump sc{ctx->ws, ctx->resident, ctx->ws_bytes};
+    double *g = sc.take<double>(M), *k = sc.take<double>(9);
+    if (!g || !k) return fail(ctx, FP_ENOMEM, "scratch");
+    CU(cudaMemcpyAsync(g, gamma_total, M * 8, cudaMemcpyHostToDevice, st));
+    launch_kappa(d, g, pref, k, st);
+    CU(cudaGetLastError());
+    CU(cudaMemcpyAsync(kappa, k, 72, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    return FP_OK;
+}
+
+// ---- debug list export -------------------------------------------------------------------------------------------------
+static int list_driver(fp_ctx *ctx, int order, int32_t target, int32_t channel, int32_t qp, int32_t *out, int64_t cap,
+                       int64_t *n, cudaStream_t st) {
+    if (!ctx || !n) return FP_EINVAL;
+    const FpDev &d = ctx->d;
+    if (!(order == 3 ? ctx->has3 : ctx->has4)) return fail(ctx, FP_ESTATE, "no IFC list of this order was given to fp_setup");
+    const int nch = order == 3 ? 2 : 3;
+    if (target < 0 || target >= d.N * d.nb || channel < 0 || channel >= nch || cap < 0 || (cap > 0 && !out))
+        return fail(ctx, FP_EINVAL, "bad target/channel/cap");
+    if (order == 4 && (qp < 0 || qp >= d.N)) return fail(ctx, FP_EINVAL, "bad q'");
+    const int64_t rows_per_unit = order == 3 ? 1 : d.nb;
+    const int64_t nrows = nch * rows_per_unit;
+    const int w = order == 3 ? 2 : 3;
+    Bump sc{ctx->ws, ctx->resident, ctx->ws_bytes};
+    int32_t *d_t = sc.take<int32_t>(1);
+    uint32_t *cnt = sc.take<uint32_t>(nrows);
+    int64_t *offs = sc.take<int64_t>(nrows + 1), *bsums = sc.take<int64_t>(16);
+    if (!d_t || !cnt || !offs || !bsums) return fail(ctx, FP_ENOMEM, "scratch");
+    CU(cudaMemcpyAsync(d_t, &target, 4, cudaMemcpyHostToDevice, st));
+    RowArgs ra; ra.targets = d_t; ra.row0 = 0; ra.qp_begin = qp; ra.nqp = 1;
+    launch_count(order, d, ra, nrows, cnt, st);
+    launch_scan(cnt, nrows, offs, bsums, st);
+    std::vector<int64_t> ho(nrows + 1);
+    CU(cudaMemcpyAsync(ho.data(), offs, (nrows + 1) * 8, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    const int64_t total = ho[nrows];
+    uint32_t *list = sc.take<uint32_t>(std::max<int64_t>(total, 1));
+    int32_t *dec = sc.take<int32_t>(std::max<int64_t>(total, 1) * w);
+    if (!list || !dec) return fail(ctx, FP_ENOMEM, "scratch");
+    launch_fill(order, d, ra, nrows, offs, 0, list, st);
+    const int64_t rb = channel * rows_per_unit, re = rb + rows_per_unit;
+    for (int64_t r = rb; r < re; r++) {
+        RowArgs rr = ra; rr.row0 = r;
+        launch_decode(order, d, rr, list + ho[r], ho[r + 1] - ho[r], dec + (ho[r] - ho[rb]) * w, st);
+    }
+    CU(cudaGetLastError());
+    *n = ho[re] - ho[rb];
+    const int64_t ncopy = std::min(*n, cap);
+    if (ncopy > 0) CU(cudaMemcpyAsync(out, dec, ncopy * w * 4, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    return FP_OK;
+}
+
+int fp_list3(fp_ctx *ctx, int32_t target, int32_t channel, int32_t *pairs, int64_t cap, int64_t *n, void *stream) {
+    return list_driver(ctx, 3, target, channel, 0, pairs, cap, n, (cudaStream_t)stream);
+}
+int fp_list4(fp_ctx *ctx, int32_t target, int32_t channel, int32_t qp, int32_t *triples, int64_t cap, int64_t *n,
+             void *stream) {
+    return list_driver(ctx, 4, target, channel, qp, triples, cap, n, (cudaStream_t)stream);
+}
+
+// ---- profiling ------------------------------------------------------------------------------------------------------------
+int fp_profile_enable(fp_ctx *ctx, int on) { if (!ctx) return FP_EINVAL; ctx->profiling = on != 0; return FP_OK; }
+
+int fp_profile_reset(fp_ctx *ctx) {
+    if (!ctx) return FP_EINVAL;
+    for (auto &e : ctx->events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+    ctx->events.clear();
+    ctx->prof = fp_profile{};
+    return FP_OK;
+}
+
+int fp_profile_get(fp_ctx *ctx, fp_profile *out) {
+    if (!ctx || !out) return FP_EINVAL;
+    fp_profile p = ctx->prof;
+    p.ms_count = p.ms_scan = p.ms_fill = p.ms_precontract = p.ms_contract = p.ms_reduce = 0;
+    p.n_count = p.n_scan = p.n_fill = p.n_precontract = p.n_contract = p.n_reduce = 0;
+    for (auto &e : ctx->events) {
+        CU(cudaEventSynchronize(e.b));
+        float ms = 0;
+        CU(cudaEventElapsedTime(&ms, e.a, e.b));
+        switch (e.cat) {
+            case CAT_COUNT: p.ms_count += ms; p.n_count++; break;
+            case CAT_SCAN: p.ms_scan += ms; p.n_scan++; break;
+            case CAT_FILL: p.ms_fill += ms; p.n_fill++; break;
+            case CAT_PRE: p.ms_precontract += ms; p.n_precontract++; break;
+            case CAT_CONTRACT: p.ms_contract += ms; p.n_contract++; break;
+            case CAT_REDUCE: p.ms_reduce += ms; p.n_reduce++; break;
+        }
+    }
+    *out = p;
+    return FP_OK;
+}
+
+int fp_probe_fp64_tflops(void *stream, double *tflops) {
+    if (!tflops) return FP_EINVAL;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+        return FP_ECUDA;
+    double t = run_fp64_probe((cudaStream_t)stream, sms);
+    if (t <= 0) return FP_ECUDA;
+    *tflops = t;
+    return FP_OK;
+}
+
+}  // extern "C"

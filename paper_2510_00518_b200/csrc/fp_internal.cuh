@@ -1,0 +1,97 @@
+// fp_internal.cuh -- shared declarations of the CUDA path (not part of the public ABI; see include/fourphonon.h).
+//
+// Notation follows SURVEY.md §8: lambda=(q,j) target, "row" = everything that is fixed while the last two legs vary:
+//   3ph row = (target, channel)            free legs A = lambda'  (q',  j'),  B = lambda''  (q''  = q + s2 q')
+//   4ph row = (target, channel, lambda')   free legs A = lambda'' (q'', j''), B = lambda''' (q''' = qbase + s2 q'')
+// A candidate inside a row is the code  (qx*nb + ja)*nb + jb  with qx the free q-point of leg A.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/fourphonon.h"
+
+#define FP_MAX_NB 64          // branch-mask width of the enumerator (natoms <= 21)
+#define FP_MAX_L 4096         // lcm of the mesh dimensions (1-D phase table in shared memory)
+
+// One mode record, 32 B: the enumerator and the weight code read omega and v_g together.
+struct __align__(32) ModeRec { double omega, vx, vy, vz; };
+
+// Device-resident tables, passed to kernels by value.
+struct FpDev {
+    int nat, nb, N, N1, N2, N3;
+    int L, m1, m2, m3;            // L = lcm(N1,N2,N3); m_mu = L/N_mu ; phase(q,R) = ph1d[(sum_mu i_mu m_mu n_mu) mod L]
+    int Lmask;                    // L-1 if L is a power of two, else -1
+    double B[9];                  // B_mu = b_mu/N_mu, pinned arithmetic
+    double scale, ncut, sigma_const, T;
+    const ModeRec *rec;           // N*nb
+    const double *occ;            // N*nb  f_lambda = 1/expm1(hbar omega/kB T)
+    const double2 *evec;          // N*nb*nb mass-scaled eigenvectors e~ = e/sqrt(m)
+    const double2 *ph1d;          // L
+    const int *qc;                // N packed mesh coordinates i1 | i2<<10 | i3<<20   (N_mu <= 1024)
+};
+
+// Anharmonic list in device layout: clusters sorted by contraction block.
+//  ORDER 3: block = (atom j, atom k, Rj-Rk);  cl_meta0 = {i, Rk}            (phase conj(phi(q,Rk)) at level 0)
+//  ORDER 4: block = (atom k, atom l, Rk-Rl);  cl_meta0 = {i, Rl}, cl_meta1 = {j, Rj-Rl}  (level 1)
+// All cell offsets are stored reduced to [0,N_mu).
+struct IfcDev {
+    int n, nblk, ncomp;           // clusters, blocks, 27 or 81
+    const int4 *cl_meta0;         // n
+    const int4 *cl_meta1;         // n (ORDER 4 only)
+    const double *phi;            // n*ncomp, block-sorted
+    const int *blk_start;         // nblk+1 (CSR over clusters)
+    const int4 *blk_meta;         // nblk {atomA | atomB<<16, d1, d2, d3}
+    const int *seg;               // nat*nat+1 : block ranges per (atomA, atomB), blocks sorted by (atomA, atomB)
+};
+
+struct RowArgs {
+    const int32_t *targets;       // device
+    int64_t row0;                 // first row handled by this launch
+    int qp_begin, nqp;            // 4ph only
+};
+
+struct EventRec { int cat; cudaEvent_t a, b; };
+
+struct fp_ctx {
+    FpDev d;
+    IfcDev i3, i4;
+    bool has3 = false, has4 = false;
+    double vol = 0;               // |a1.(a2 x a3)|
+    char *ws = nullptr;           // caller workspace
+    size_t ws_bytes = 0, resident = 0;   // resident tables occupy [0, resident)
+    int sm_count = 148;
+    bool profiling = false;
+    std::vector<EventRec> events;
+    std::vector<cudaEvent_t> pool;
+    fp_profile prof{};
+    std::string err;
+    void *pinned = nullptr;       // small pinned staging buffer
+    size_t pinned_bytes = 0;
+};
+
+enum { CAT_COUNT = 0, CAT_SCAN, CAT_FILL, CAT_PRE, CAT_CONTRACT, CAT_REDUCE };
+
+// ---- kernel launchers (fp_kernels.cu) --------------------------------------------------------------------------------
+void launch_tables(const FpDev &d, const double *omega, const double *eig, const double *vg, const double *masses_dev,
+                   double hbar_over_kb, ModeRec *rec, double *occ, double2 *evec, double2 *ph1d, int *qc, cudaStream_t st);
+void launch_count(int order, const FpDev &d, const RowArgs &ra, int64_t nrows, uint32_t *counts, cudaStream_t st);
+void launch_scan(const uint32_t *counts, int64_t n, int64_t *offsets /*n+1*/, int64_t *block_sums, cudaStream_t st);
+void launch_plan(const int64_t *offsets, int64_t nrows, int64_t cap, int64_t *plan /*[0]=nchunks, then bounds*/,
+                 int max_chunks, cudaStream_t st);
+void launch_fill(int order, const FpDev &d, const RowArgs &ra, int64_t nrows, const int64_t *offsets, int64_t list_base,
+                 uint32_t *list, cudaStream_t st);
+void launch_pre3(const FpDev &d, const IfcDev &f, const int32_t *targets, int64_t nt, double2 *mhat, cudaStream_t st);
+void launch_pre4(const FpDev &d, const IfcDev &f, const int32_t *targets, int64_t nt, double2 *t0, cudaStream_t st);
+void launch_contract(int order, const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const int64_t *offsets,
+                     int64_t list_base, const uint32_t *list, const double2 *pre, double2 *partial, cudaStream_t st);
+void launch_finalize(int order, const FpDev &d, const int32_t *targets, int64_t nt, int64_t rows_per_unit,
+                     const double2 *partial, const uint32_t *counts, double c_over_n, double *gamma, double *wp,
+                     int64_t *cnt, cudaStream_t st);
+void launch_kappa(const FpDev &d, const double *gamma_total, double pref, double *kappa, cudaStream_t st);
+void launch_decode(int order, const FpDev &d, const RowArgs &ra, const uint32_t *list, int64_t n, int32_t *out,
+                   cudaStream_t st);
+double run_fp64_probe(cudaStream_t st, int sm_count);
+size_t contract_smem_bytes(const FpDev &d, const IfcDev &f);

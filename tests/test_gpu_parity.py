@@ -1,0 +1,265 @@
+"""-m gpu: the CUDA path (through the C ABI of include/fourphonon.h) against the CPU oracle, element by element.
+
+Bars (BASELINE.json north_star): process counts bit-exact, rates / weighted phase space / kappa within 1e-9 relative.
+See assert_rates_close for how "relative" is measured for modes whose rate is cancellation noise.
+"""
+import numpy as np
+import pytest
+
+import fp_inputs
+
+pytestmark = pytest.mark.gpu
+
+RTOL = 1e-9
+
+
+@pytest.fixture(scope="module")
+def fp():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import paper_2510_00518_b200 as fp
+    fp.load_library()
+    return fp
+
+
+def _oracle(inp, **kw):
+    from oracle.oracle import Oracle
+    return Oracle(inp, **kw)
+
+
+def assert_rates_close(got, ref, what):
+    """|got - ref| <= 1e-9 * (largest |ref| of the channel) everywhere, and <= 1e-9 * |ref| itself wherever the mode's
+    value is not cancellation noise (|ref| >= 1e-10 of the channel maximum: below that |V|^2 is the square of a sum
+    that cancels to < 1e-5 of its terms, and no FP64 evaluation order reproduces another to 1e-9 of the result)."""
+    got = np.asarray(got); ref = np.asarray(ref)
+    assert got.shape == ref.shape
+    scale = np.abs(ref).max(axis=0, keepdims=True)
+    scale = np.where(scale > 0, scale, 1.0)
+    err = np.abs(got - ref) / scale
+    assert err.max() <= RTOL, f"{what}: max error relative to the channel maximum {err.max():.3e}"
+    big = np.abs(ref) >= 1e-10 * scale
+    if big.any():
+        own = np.abs(got[big] - ref[big]) / np.abs(ref[big])
+        assert own.max() <= RTOL, f"{what}: max error relative to own magnitude {own.max():.3e}"
+    assert np.all(got[ref == 0] == 0.0), f"{what}: oracle zero where the GPU is nonzero"
+
+
+def check3(fp, inp, targets, **kw):
+    orc = _oracle(inp, **{k: v for k, v in kw.items() if k in ("ncut", "sigma_const", "T", "scale")})
+    og, ow, oc = orc.rates3(targets)
+    with fp.Context.from_inputs(inp, scratch_bytes=kw.pop("scratch_bytes", 64 << 20), **kw) as ctx:
+        g, w, c = ctx.rates3(targets)
+    assert np.array_equal(c, oc), "3ph process counts are not bit-exact"
+    assert_rates_close(g, og, "Gamma3")
+    assert_rates_close(w, ow, "WP3")
+    return g, c
+
+
+def check4(fp, inp, targets, qp=(0, None), **kw):
+    orc = _oracle(inp, **{k: v for k, v in kw.items() if k in ("ncut", "sigma_const", "T", "scale")})
+    og, ow, oc = orc.rates4(targets, qp[0], qp[1])
+    with fp.Context.from_inputs(inp, scratch_bytes=kw.pop("scratch_bytes", 64 << 20), **kw) as ctx:
+        g, w, c = ctx.rates4(targets, qp[0], qp[1])
+    assert np.array_equal(c, oc), "4ph process counts are not bit-exact"
+    assert_rates_close(g, og, "Gamma4")
+    assert_rates_close(w, ow, "WP4")
+    return g, c
+
+
+# ---- small cases: whole job element by element ----------------------------------------------------------------------------
+def test_constants_match_oracle(fp):
+    from oracle.oracle import Oracle
+    a, b = fp.fp_constants(), Oracle.constants()
+    for k in a:
+        assert abs(a[k] - b[k]) <= 1e-14 * abs(b[k])
+
+
+@pytest.mark.parametrize("kind,mesh", [("diamond", (3, 3, 3)), ("diamond", (4, 3, 2)), ("sc1", (5, 4, 3)),
+                                       ("sc8", (2, 3, 2))])
+def test_rates3_small(fp, kind, mesh):
+    inp = fp_inputs.make_tiny(kind, mesh=mesh, with4=False)
+    g, c = check3(fp, inp, inp.targets3)
+    assert c.sum() > 0
+
+
+def test_rates3_config0_all_modes(fp):
+    inp = fp_inputs.make_config(0)["main"]
+    g, c = check3(fp, inp, inp.targets3)
+    assert c.sum() > 1e5
+
+
+@pytest.mark.parametrize("kind,mesh,sl", [("diamond", (3, 3, 3), slice(5, 29)), ("diamond", (4, 2, 3), slice(40, 52)),
+                                          ("sc1", (4, 3, 3), slice(0, None))])
+def test_rates4_small(fp, kind, mesh, sl):
+    inp = fp_inputs.make_tiny(kind, mesh=mesh)
+    g, c = check4(fp, inp, inp.targets4[sl])
+    assert c.sum() > 0
+
+
+def test_rates4_many_branch_generic_path(fp):
+    inp = fp_inputs.make_tiny("sc8", mesh=(2, 2, 3))
+    check4(fp, inp, inp.targets4[30:36], qp=(3, 7))
+
+
+def test_filter_disabled_constant_sigma_2x2x2(fp):
+    """item 20: adaptive sigma vanishes on 2x2x2, so the brute-force configuration is ncut=inf with a fixed sigma."""
+    inp = fp_inputs.make_tiny("diamond", mesh=(2, 2, 2))
+    g3, c3 = check3(fp, inp, inp.targets3, ncut=float("inf"), sigma_const=5.0)
+    nb, N = inp.nb, inp.nq
+    for i, lam in enumerate(inp.targets3):
+        expect = 0 if inp.omega.reshape(-1)[lam] == 0.0 else N * nb * nb - 6 * nb + (9 if lam // nb == 0 else 0)
+        assert c3[i, 0] == expect and c3[i, 1] == expect
+    check4(fp, inp, inp.targets4[3:15], ncut=float("inf"), sigma_const=5.0)
+
+
+def test_adaptive_sigma_on_2x2x2_rejects_everything(fp):
+    inp = fp_inputs.make_tiny("diamond", mesh=(2, 2, 2), with4=False)
+    g, c = check3(fp, inp, inp.targets3)
+    assert c.sum() == 0 and np.all(g == 0.0)
+
+
+def test_list3_equals_oracle_list_as_sets(fp):
+    inp = fp_inputs.make_tiny("diamond", mesh=(4, 4, 4), with4=False)
+    orc = _oracle(inp)
+    with fp.Context.from_inputs(inp, scratch_bytes=32 << 20) as ctx:
+        for lam in (7, 100, 383):
+            for ch in (0, 1):
+                a = ctx.list3(lam, ch); b = orc.list3(lam, ch)
+                assert len(a) == len(b)
+                assert set(map(tuple, a.tolist())) == set(map(tuple, b.tolist()))
+
+
+def test_list4_is_momentum_conserving_and_counts_match(fp):
+    inp = fp_inputs.make_tiny("diamond", mesh=(3, 3, 3))
+    orc = _oracle(inp)
+    coords = fp_inputs.qpoint_coords(inp.mesh)
+    nb = inp.nb
+    lam = 31
+    with fp.Context.from_inputs(inp, scratch_bytes=32 << 20) as ctx:
+        for ch, (s1, s2) in enumerate(((1, 1), (1, -1), (-1, -1))):
+            for qp in (0, 5, 26):
+                tr = ctx.list4(lam, ch, qp)
+                _, _, oc = orc.rates4(np.array([lam], dtype=np.int32), qp, qp + 1)
+                assert len(tr) == oc[0, ch]
+                assert len(set(map(tuple, tr.tolist()))) == len(tr)
+                for l1, l2, l3 in tr:
+                    assert l1 // nb == qp
+                    q3 = (coords[lam // nb] + s1 * coords[l1 // nb] + s2 * coords[l2 // nb]) % inp.mesh
+                    assert np.array_equal(q3, coords[l3 // nb])
+
+
+# ---- boundary behaviour ------------------------------------------------------------------------------------------------------
+def test_device_pointer_entry_points_match_host_entry_points(fp):
+    import torch
+    inp = fp_inputs.make_tiny("diamond", mesh=(3, 3, 3))
+    dev = torch.device("cuda:0")
+    om = torch.from_numpy(np.ascontiguousarray(inp.omega)).to(dev)
+    eg = torch.from_numpy(np.ascontiguousarray(inp.eig)).to(dev)
+    vg = torch.from_numpy(np.ascontiguousarray(inp.vg)).to(dev)
+    with fp.Context.from_inputs(inp, scratch_bytes=32 << 20) as a, \
+            fp.Context(inp.crystal.lattvec, inp.crystal.masses, om, eg, vg, inp.mesh, T=inp.T, ifc3=inp.ifc3,
+                       ifc4=inp.ifc4, scratch_bytes=32 << 20) as b:
+        t3 = inp.targets3
+        g, w, c = a.rates3(t3)
+        gd, wd, cd = b.rates3(torch.from_numpy(t3).to(dev))
+        assert np.array_equal(g, gd.cpu().numpy()) and np.array_equal(w, wd.cpu().numpy())
+        assert np.array_equal(c, cd.cpu().numpy())
+        t4 = inp.targets4[10:16]
+        g4, w4, c4 = a.rates4(t4)
+        g4d, w4d, c4d = b.rates4(torch.from_numpy(t4).to(dev))
+        assert np.array_equal(g4, g4d.cpu().numpy()) and np.array_equal(c4, c4d.cpu().numpy())
+        k = a.kappa_rta(g.sum(axis=1))
+        kd = b.kappa_rta(gd.sum(dim=1))
+        assert np.array_equal(k, kd.cpu().numpy())
+
+
+def test_rates4_partial_q_ranges_add_up(fp):
+    inp = fp_inputs.make_tiny("diamond", mesh=(3, 3, 3))
+    t = inp.targets4[20:26]
+    with fp.Context.from_inputs(inp, scratch_bytes=32 << 20) as ctx:
+        g, w, c = ctx.rates4(t)
+        ga, wa, ca = ctx.rates4(t, 0, 11)
+        gb, wb, cb = ctx.rates4(t, 11, 27)
+        ge, we, ce = ctx.rates4(t, 5, 5)
+    assert np.array_equal(c, ca + cb)
+    assert np.allclose(g, ga + gb, rtol=1e-12, atol=0)
+    assert np.all(ge == 0) and np.all(ce == 0)
+
+
+def test_chunked_lists_give_identical_results(fp):
+    """A scratch just above the minimum forces many list chunks (Algorithm 5's mode-by-mode regime)."""
+    inp = fp_inputs.make_config(0)["main"]
+    t = inp.targets3[:96]
+    with fp.Context.from_inputs(inp, scratch_bytes=64 << 20) as big:
+        g, w, c = big.rates3(t)
+    with fp.Context.from_inputs(inp, scratch_bytes=160 << 10) as small:
+        small.profile_enable(True)
+        gs, ws, cs = small.rates3(t)
+        assert small.profile_get().chunks > 1
+    assert np.array_equal(c, cs) and np.array_equal(g, gs) and np.array_equal(w, ws)
+
+
+def test_run_to_run_determinism(fp):
+    inp = fp_inputs.make_tiny("diamond", mesh=(3, 3, 3))
+    with fp.Context.from_inputs(inp, scratch_bytes=32 << 20) as ctx:
+        a = ctx.rates4(inp.targets4[6:12])
+        b = ctx.rates4(inp.targets4[6:12])
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y)
+
+
+def test_empty_and_zero_mode_targets(fp):
+    inp = fp_inputs.make_tiny("diamond", mesh=(3, 3, 3))
+    with fp.Context.from_inputs(inp, scratch_bytes=32 << 20) as ctx:
+        g, w, c = ctx.rates3(np.zeros(0, dtype=np.int32))
+        assert g.shape == (0, 2)
+        g, w, c = ctx.rates3(np.array([0, 1, 2], dtype=np.int32))          # the three Gamma acoustic modes
+        assert np.all(g == 0) and np.all(w == 0) and np.all(c == 0)
+        g, w, c = ctx.rates4(np.array([0, 1, 2], dtype=np.int32))
+        assert np.all(g == 0) and np.all(w == 0) and np.all(c == 0)
+
+
+def test_error_codes(fp):
+    inp = fp_inputs.make_tiny("diamond", mesh=(3, 3, 3), with4=False)
+    with fp.Context.from_inputs(inp, scratch_bytes=32 << 20) as ctx:
+        with pytest.raises(fp.FourPhononError) as e:
+            ctx.rates4(inp.targets4[:2])
+        assert e.value.code == fp.FP_ESTATE
+        with pytest.raises(fp.FourPhononError) as e:
+            ctx.rates3(np.array([inp.nq * inp.nb], dtype=np.int32))
+        assert e.value.code == fp.FP_EINVAL
+        with pytest.raises(fp.FourPhononError) as e:
+            ctx.rates3(np.array([-1], dtype=np.int32))
+        assert e.value.code == fp.FP_EINVAL
+    with pytest.raises(fp.FourPhononError) as e:
+        fp.Context.from_inputs(inp, T=0.0)
+    assert e.value.code == fp.FP_EINVAL
+    with pytest.raises(fp.FourPhononError) as e:
+        fp.Context.from_inputs(inp, scale=-1.0)
+    assert e.value.code == fp.FP_EINVAL
+    bad = np.array(inp.omega, copy=True); bad.reshape(-1)[10] = float("nan")
+    with pytest.raises(fp.FourPhononError) as e:
+        fp.Context(inp.crystal.lattvec, inp.crystal.masses, bad, inp.eig, inp.vg, inp.mesh, ifc3=inp.ifc3)
+    assert e.value.code == fp.FP_EINVAL
+    atoms = np.array(inp.ifc3[0], copy=True); atoms[0, 1] = 7
+    with pytest.raises(fp.FourPhononError) as e:
+        fp.Context(inp.crystal.lattvec, inp.crystal.masses, inp.omega, inp.eig, inp.vg, inp.mesh,
+                   ifc3=(atoms, inp.ifc3[1], inp.ifc3[2]))
+    assert e.value.code == fp.FP_EINVAL
+    with pytest.raises(fp.FourPhononError) as e:                           # scratch below one row of candidates
+        with fp.Context.from_inputs(inp, scratch_bytes=1) as ctx:
+            ctx.rates3(inp.targets3[:4])
+    assert e.value.code == fp.FP_ENOMEM
+
+
+def test_kappa_matches_oracle(fp):
+    inp = fp_inputs.make_config(0)["main"]
+    orc = _oracle(inp)
+    with fp.Context.from_inputs(inp, scratch_bytes=64 << 20) as ctx:
+        g, w, c = ctx.rates3(inp.targets3)
+        gt = g.sum(axis=1)
+        k = ctx.kappa_rta(gt)
+    ok = orc.kappa(gt)
+    assert np.abs(k - ok).max() <= RTOL * np.abs(ok).max()
+    assert np.allclose(k, k.T, rtol=1e-12, atol=1e-12 * np.abs(k).max())    # symmetric by construction
