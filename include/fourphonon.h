@@ -25,9 +25,9 @@
  *
  * Execution
  *   All kernels and copies are issued on `stream` (a cudaStream_t passed as void*, NULL = default stream).
- *   fp_setup, fp_rates3 and fp_rates4 synchronise the stream internally (chunk planning reads a few bytes of
- *   device-side counts back; Algorithm 5 is the same mode-by-mode host loop), so on return the
- *   outputs are complete.  fp_kappa_rta with FP_MEM_DEVICE outputs is asynchronous.
+ *   fp_setup, fp_rates3 and fp_rates4 synchronise the stream before returning (the scratch region is reused by the
+ *   next super-chunk of targets, the bounded-memory loop of Algorithm 5), so on return the outputs
+ *   are complete.  fp_kappa_rta with FP_MEM_DEVICE outputs is asynchronous.
  *
  * Errors
  *   Every call returns FP_OK (0) or a negative code; nothing throws or aborts.  fp_last_error(ctx) (ctx may be NULL
@@ -77,16 +77,18 @@ typedef struct {
 
 /* Device-time profile of the kernels launched since the last fp_profile_reset (CUDA events on the launch stream).   */
 typedef struct {
-    double  ms_count, ms_scan, ms_fill, ms_precontract, ms_contract, ms_reduce;  /* summed launch durations, ms     */
-    int64_t n_count, n_scan, n_fill, n_precontract, n_contract, n_reduce;        /* launches                        */
-    int64_t candidates;     /* momentum-conserving candidates examined by the count pass                            */
-    int64_t processes;      /* allowed processes evaluated by the contraction kernels                               */
-    double  contract_flops; /* FP64 flops executed by the contraction kernels (analytic model)        */
-    int64_t chunks;         /* list chunks                                                                          */
+    double  ms_precontract, ms_rates, ms_reduce;      /* summed launch durations, ms: per-target pre-contraction,     */
+    int64_t n_precontract, n_rates, n_reduce;         /* fused enumerate+evaluate kernel, per-mode reduction; launches */
+    int64_t rows;           /* rows ((target, channel[, lambda']) units, one CTA each) of the fused kernel               */
+    int64_t candidates;     /* momentum-conserving candidates examined by the enumerator                            */
+    int64_t prefiltered;    /* candidates admitted by the FP32 pre-filter (superset of the allowed ones)            */
+    int64_t processes;      /* allowed processes (pinned FP64 decision) evaluated                                   */
+    double  rates_flops;    /* FP64 flops of the per-process contraction (analytic model)             */
 } fp_profile;
 
-/* Bytes of workspace fp_setup needs for its resident tables plus `scratch_bytes` of per-call scratch (row arrays +
- * process-list buffer; larger scratch = fewer chunks).  ifc3/ifc4 may be NULL.  Returns 0 on invalid arguments.     */
+/* Bytes of workspace fp_setup needs for its resident tables plus `scratch_bytes` of per-call scratch (per-target
+ * pre-contracted tables and 20 bytes per row of partial sums; a larger scratch means fewer launches).  ifc3/ifc4 may
+ * be NULL.  Returns 0 on invalid arguments.                                                                         */
 size_t fp_workspace_bytes(const fp_crystal *crystal, const int32_t mesh[3], const fp_ifc *ifc3, const fp_ifc *ifc4,
                           size_t scratch_bytes);
 
@@ -98,7 +100,8 @@ size_t fp_workspace_bytes(const fp_crystal *crystal, const int32_t mesh[3], cons
  *   vg       loc  N*nb*3          (Angstrom/ps)
  *   ifc3, ifc4 may be NULL (then fp_rates3 / fp_rates4 return FP_ESTATE)
  * Errors: FP_EINVAL for mesh <= 0, natoms <= 0 or > 21, NaN/negative omega, 0 < omega < 1e-6*omega_max, T <= 0,
- * scale <= 0, ncut < 0, atom index out of range, lcm(N1,N2,N3) > 4096; FP_ENOMEM if workspace_bytes is too small.  */
+ * scale <= 0, ncut < 0, atom index out of range, lcm(N1,N2,N3) > 4096, more than 2^20 q-points; FP_ENOMEM if
+ * workspace_bytes is too small.                                                                                    */
 int fp_setup(const fp_crystal *crystal, const double *masses, const double *omega, const double *eig, const double *vg,
              fp_memloc mode_arrays_loc, const fp_ifc *ifc3, const fp_ifc *ifc4, const int32_t mesh[3], double T,
              const fp_broadening *broadening, void *workspace, size_t workspace_bytes, void *stream, fp_ctx **out);

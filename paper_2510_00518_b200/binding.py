@@ -22,7 +22,7 @@ FP_MEM_HOST, FP_MEM_DEVICE = 0, 1
 _PKG = Path(__file__).resolve().parent
 _CSRC = _PKG / "csrc"
 _LIB = _PKG / "libfourphonon_b200.so"
-_SOURCES = ["fp_kernels.cu", "fp_host.cu"]
+_SOURCES = ["fp_kernels.cu", "fp_rates.cu", "fp_host.cu"]
 
 # every symbol include/fourphonon.h declares (tests check that the built library exports all of them)
 EXPORTED_SYMBOLS = [
@@ -45,7 +45,7 @@ def library_path() -> Path:
 def build_library(force: bool = False, verbose: bool = False) -> Path:
     """nvcc -gencode arch=compute_100a,code=sm_100a (cross-compiles without a GPU); in-tree so it ships with gpurun."""
     srcs = [_CSRC / s for s in _SOURCES]
-    deps = srcs + [_CSRC / "fp_internal.cuh", _PKG.parent / "include" / "fourphonon.h"]
+    deps = srcs + [_CSRC / "fp_internal.cuh", _CSRC / "fp_device.cuh", _PKG.parent / "include" / "fourphonon.h"]
     if not force and _LIB.exists() and all(_LIB.stat().st_mtime >= d.stat().st_mtime for d in deps):
         return _LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
@@ -70,33 +70,28 @@ class _Broadening(C.Structure):
 
 
 class _Profile(C.Structure):
-    _fields_ = [(n, C.c_double) for n in ("ms_count", "ms_scan", "ms_fill", "ms_precontract", "ms_contract", "ms_reduce")] + \
-               [(n, C.c_int64) for n in ("n_count", "n_scan", "n_fill", "n_precontract", "n_contract", "n_reduce")] + \
-               [("candidates", C.c_int64), ("processes", C.c_int64), ("contract_flops", C.c_double), ("chunks", C.c_int64)]
+    _fields_ = [(n, C.c_double) for n in ("ms_precontract", "ms_rates", "ms_reduce")] + \
+               [(n, C.c_int64) for n in ("n_precontract", "n_rates", "n_reduce", "rows", "candidates", "prefiltered",
+                                         "processes")] + [("rates_flops", C.c_double)]
 
 
 @dataclass
 class Profile:
-    ms_count: float
-    ms_scan: float
-    ms_fill: float
     ms_precontract: float
-    ms_contract: float
+    ms_rates: float
     ms_reduce: float
-    n_count: int
-    n_scan: int
-    n_fill: int
     n_precontract: int
-    n_contract: int
+    n_rates: int
     n_reduce: int
+    rows: int
     candidates: int
+    prefiltered: int
     processes: int
-    contract_flops: float
-    chunks: int
+    rates_flops: float
 
     @property
     def launches(self) -> int:
-        return self.n_count + self.n_scan + self.n_fill + self.n_precontract + self.n_contract + self.n_reduce
+        return self.n_precontract + self.n_rates + self.n_reduce
 
 
 _lib = None
@@ -195,7 +190,7 @@ class Context:
     """fp_setup ... fp_destroy.  Owns the device workspace (a torch uint8 CUDA tensor) for the context's lifetime."""
 
     def __init__(self, lattvec, masses, omega, eig, vg, mesh, T=300.0, ifc3=None, ifc4=None, scale=1.0, ncut=2.0,
-                 sigma_const=0.0, scratch_bytes=1 << 30, device="cuda:0", stream=None):
+                 sigma_const=0.0, scratch_bytes=1 << 30, device="cuda:0", stream=None, workspace_bytes=None):
         import torch
         self._torch = torch
         self.lib = load_library()
@@ -244,6 +239,8 @@ class Context:
         nbytes = self.lib.fp_workspace_bytes(C.byref(cr), mesh_c, p3, p4, int(scratch_bytes))
         if nbytes == 0:
             raise FourPhononError(FP_EINVAL, "fp_workspace_bytes rejected the arguments")
+        if workspace_bytes is not None:                                # caller-chosen size (fp_setup checks it)
+            nbytes = int(workspace_bytes)
         with torch.cuda.device(self.device):
             self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
             off = (-self.workspace.data_ptr()) % 256

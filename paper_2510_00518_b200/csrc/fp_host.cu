@@ -1,5 +1,5 @@
 // fp_host.cu -- host side of the C ABI (include/fourphonon.h): argument checking, IFC block analysis, workspace
-// carving, chunk planning (Algorithm 5's mode-by-mode loop, generalised to list chunks) and launches.
+// carving, the bounded-memory loop over super-chunks of targets (Algorithm 5) and launches.
 // All arithmetic of the method runs in the kernels of fp_kernels.cu; the only floating-point work here is the 3x3
 // reciprocal-lattice setup B_mu = b_mu/N_mu in the pinned order of SURVEY.md §8(c) step 3 and the unit constants.
 #include <algorithm>
@@ -132,8 +132,8 @@ size_t ifc_resident_bytes(int64_t n, int order, int nat) {
 
 size_t tables_resident_bytes(int nat, const int32_t mesh[3], long L) {
     size_t N = (size_t)mesh[0] * mesh[1] * mesh[2], nb = 3 * (size_t)nat, M = N * nb;
-    return align_up(M * sizeof(ModeRec)) + align_up(M * 8) + align_up(M * nb * 16) + align_up((size_t)L * 16) +
-           align_up(N * 4) + align_up(nat * 8) + 256 * 8;
+    return align_up(M * sizeof(ModeRec)) + align_up(M * 16) + align_up(M * 8) + align_up(M * nb * 16) +
+           align_up((size_t)L * 16) + align_up(N * 4) + align_up(nat * 8) + 256 * 10;
 }
 
 long mesh_lcm(const int32_t mesh[3]) {
@@ -226,8 +226,8 @@ int fp_setup(const fp_crystal *crystal, const double *masses, const double *omeg
     const long L = mesh_lcm(mesh);
     if (L > FP_MAX_L) return fail(ctx, FP_EINVAL, "lcm of the mesh dimensions exceeds 4096");
     const size_t N = (size_t)mesh[0] * mesh[1] * mesh[2], nb = 3 * (size_t)nat, M = N * nb;
-    if (M * nb > (size_t)1 << 31 || N * nb * nb > (size_t)0xffffffffu)
-        return fail(ctx, FP_EINVAL, "mesh * branches too large for 32-bit candidate codes");
+    if (M * nb > (size_t)1 << 31 || N > (size_t)1 << 20)
+        return fail(ctx, FP_EINVAL, "more than 2^20 q-points (32-bit candidate codes)");
     if ((reinterpret_cast<uintptr_t>(workspace) & 255) != 0) return fail(ctx, FP_EINVAL, "workspace must be 256-byte aligned");
 
     IfcHost h3, h4;
@@ -280,15 +280,17 @@ int fp_setup(const fp_crystal *crystal, const double *masses, const double *omeg
     // ---- carve resident tables -----------------------------------------------------------------------------------
     Bump bump{ctx->ws, 0, workspace_bytes};
     ModeRec *rec = bump.take<ModeRec>(M);
+    float4 *recf = bump.take<float4>(M);
+    unsigned long long *maxima = bump.take<unsigned long long>(2);
     double *occ = bump.take<double>(M);
     double2 *evec = bump.take<double2>(M * nb);
     double2 *ph1d = bump.take<double2>(L);
     int *qc = bump.take<int>(N);
     double *masses_dev = bump.take<double>(nat);
-    if (!rec || !occ || !evec || !ph1d || !qc || !masses_dev) {
+    if (!rec || !recf || !maxima || !occ || !evec || !ph1d || !qc || !masses_dev) {
         fail(ctx, FP_ENOMEM, "workspace too small for the mode tables"); return bail(FP_ENOMEM);
     }
-    d.rec = rec; d.occ = occ; d.evec = evec; d.ph1d = ph1d; d.qc = qc;
+    d.rec = rec; d.recf = recf; d.occ = occ; d.evec = evec; d.ph1d = ph1d; d.qc = qc;
     if (ifc3) { int rc = upload_ifc(ctx, bump, h3, ctx->i3, st); if (rc) return bail(rc); ctx->has3 = true; }
     if (ifc4) { int rc = upload_ifc(ctx, bump, h4, ctx->i4, st); if (rc) return bail(rc); ctx->has4 = true; }
     ctx->resident = align_up(bump.off);
@@ -321,9 +323,31 @@ int fp_setup(const fp_crystal *crystal, const double *masses, const double *omeg
             return bail(FP_EINVAL);
         }
     CU(cudaMemcpyAsync(masses_dev, masses, nat * 8, cudaMemcpyHostToDevice, st));
-    launch_tables(d, d_omega, d_eig, d_vg, masses_dev, hbar_over_kb(), rec, occ, evec, ph1d, qc, st);
+    launch_tables(d, d_omega, d_eig, d_vg, masses_dev, hbar_over_kb(), rec, recf, occ, evec, ph1d, qc, maxima, st);
     CU(cudaGetLastError());
+    unsigned long long hmax[2] = {0, 0};
+    CU(cudaMemcpyAsync(hmax, maxima, sizeof(hmax), cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
+    {   // FP32 pre-filter constants: every candidate the pinned FP64 decision allows satisfies
+        //   Delta_f^2 <= pfK1 * |u_a - u_b|_f^2 + pfC2   in FP32 arithmetic on the FP32-rounded table.
+        double omax, umax;
+        std::memcpy(&omax, &hmax[0], 8); std::memcpy(&umax, &hmax[1], 8);
+        const double eta = 1e-2;                                      // 2 delta r <= eta r^2 + delta^2/eta
+        const double da = 1e-6 * omax;                                // |Delta_f - Delta|  (bound 6.6e-7 omega_max)
+        double K1, C2;
+        if (d.sigma_const > 0.0) {
+            const double r = d.ncut * d.sigma_const * (1.0 + 1e-6) + da;
+            K1 = 0.0; C2 = r * r * (1.0 + 1e-5);
+        } else {
+            const double cs = d.ncut * d.scale / std::sqrt(6.0);
+            const double dr = cs * 1e-6 * umax;                       // | |u_a-u_b|_f - |u_a-u_b| | (bound 4.2e-7 u_max)
+            const double dd = da + dr;
+            K1 = cs * cs * (1.0 + eta + 1e-5); C2 = dd * dd * (1.0 + 1.0 / eta) * (1.0 + 1e-5);
+        }
+        if (!(K1 < 1e30) || !(C2 < 1e30)) { K1 = 0.0; C2 = INFINITY; }  // filter disabled (ncut = inf): admit everything
+        d.pfK1 = std::nextafterf((float)K1, INFINITY);
+        d.pfC2 = std::isinf(C2) ? INFINITY : std::nextafterf((float)C2, INFINITY);
+    }
     *out = ctx;
     return FP_OK;
 #undef CU
@@ -344,6 +368,9 @@ int fp_destroy(fp_ctx *ctx) {
 }
 
 // ---- shared driver of fp_rates3 / fp_rates4 ------------------------------------------------------------------------------
+// Rows (3ph: (target, channel); 4ph: (target, channel, lambda')) are independent: one launch of the fused kernel per
+// super-chunk of targets whose per-row partial sums fit the scratch (Algorithm 5's bounded-memory loop, PAPER.md:354-393,
+// with chunks of many modes instead of one), then the fixed-order per-mode reduction.
 static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t nt, int32_t qp_begin, int32_t qp_end,
                         double *gamma, double *wp, int64_t *counts, fp_memloc loc, cudaStream_t st) {
     if (!ctx) return FP_EINVAL;
@@ -376,20 +403,19 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
         CU(cudaStreamSynchronize(st));
         return FP_OK;
     }
+    if (rates_smem_bytes(d, f) > 227 * 1024 - 1024)
+        return fail(ctx, FP_ENOMEM, "IFC block table exceeds the shared memory of one SM");
 
-    // ---- scratch budget: per-target arrays for a super-chunk of targets + one list buffer -----------------------------
+    // ---- scratch budget: per-target arrays for a super-chunk of targets ------------------------------------------------
     const size_t scratch = ctx->ws_bytes - ctx->resident;
     const size_t pre_per_target = (order == 3 ? (size_t)f.nblk * 9 : (size_t)f.n * 27) * sizeof(double2);
-    const size_t per_target = pre_per_target + (size_t)rows_per_target * (4 + 8 + 16) + (size_t)nch * 24 + 4 + 64;
-    const size_t fixed = 64 * 1024 + (size_t)(rows_per_target / 1024 + 16) * 8;
-    const size_t list_min = (size_t)row_cands * 4;
-    if (scratch < fixed + list_min + per_target + 8192) return fail(ctx, FP_ENOMEM, "workspace scratch too small for one target");
-    int64_t nts_max = (int64_t)std::min<size_t>((size_t)nt, std::max<size_t>(1, (scratch / 2) / per_target));
-    while (nts_max > 1 && fixed + list_min + (size_t)nts_max * per_target + 65536 > scratch) nts_max /= 2;
+    const size_t per_target = pre_per_target + (size_t)rows_per_target * (4 + 16) + (size_t)nch * 24 + 4 + 64;
+    const size_t fixed = 16 * 1024;
+    if (scratch < fixed + per_target) return fail(ctx, FP_ENOMEM, "workspace scratch too small for one target");
+    int64_t nts_max = (int64_t)std::min<size_t>((size_t)nt, (scratch - fixed) / per_target);
     while (nts_max * rows_per_target > (int64_t)1 << 30) nts_max = std::max<int64_t>(1, nts_max / 2);
 
     const double c_over_n = order == 3 ? const_c3() / (double)d.N : const_c4() / ((double)d.N * (double)d.N);
-    const int max_chunks = 4096;
 
     for (int64_t t0 = 0; t0 < nt; t0 += nts_max) {
         const int64_t nts = std::min(nts_max, nt - t0);
@@ -404,71 +430,45 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
         }
         double2 *pre = sc.take<double2>(nts * (pre_per_target / sizeof(double2)));
         uint32_t *cnt = sc.take<uint32_t>(nrows);
-        int64_t *offs = sc.take<int64_t>(nrows + 1);
-        int64_t *bsums = sc.take<int64_t>(nrows / 4096 + 8);
         double2 *partial = sc.take<double2>(nrows);
-        int64_t *plan = sc.take<int64_t>(max_chunks + 1);
-        double *o_gamma = nullptr, *o_wp = nullptr; int64_t *o_cnt = nullptr;
-        if (loc == FP_MEM_HOST || !wp || !counts) {
-            o_gamma = sc.take<double>(nts * nch); o_wp = sc.take<double>(nts * nch); o_cnt = sc.take<int64_t>(nts * nch);
-            if (!o_gamma || !o_wp || !o_cnt) return fail(ctx, FP_ENOMEM, "scratch");
-        }
-        if (!pre || !cnt || !offs || !bsums || !partial || !plan) return fail(ctx, FP_ENOMEM, "scratch");
-        const int64_t cap = (int64_t)(sc.left() / 4) - 64;
-        if (cap < row_cands) return fail(ctx, FP_ENOMEM, "workspace scratch too small for the process list");
-        uint32_t *list = sc.take<uint32_t>(cap);
+        unsigned long long *stat = sc.take<unsigned long long>(1);
+        double *o_gamma = sc.take<double>(nts * nch), *o_wp = sc.take<double>(nts * nch);
+        int64_t *o_cnt = sc.take<int64_t>(nts * nch);
+        if (!pre || !cnt || !partial || !stat || !o_gamma || !o_wp || !o_cnt) return fail(ctx, FP_ENOMEM, "scratch");
 
         RowArgs ra; ra.targets = d_targets; ra.row0 = 0; ra.qp_begin = qp_begin; ra.nqp = (int)nqp;
+        ra.prefiltered = ctx->profiling ? stat : nullptr;
+        if (ctx->profiling) CU(cudaMemsetAsync(stat, 0, sizeof(unsigned long long), st));
         { ProfScope p(ctx, CAT_PRE, st);
           if (order == 3) launch_pre3(d, f, d_targets, nts, pre, st); else launch_pre4(d, f, d_targets, nts, pre, st); }
         CU(cudaGetLastError());
-        { ProfScope p(ctx, CAT_COUNT, st); launch_count(order, d, ra, nrows, cnt, st); }
-        CU(cudaGetLastError());
-        { ProfScope p(ctx, CAT_SCAN, st); launch_scan(cnt, nrows, offs, bsums, st); launch_plan(offs, nrows, cap, plan, max_chunks, st); }
-        CU(cudaGetLastError());
-        int64_t *hplan = (int64_t *)ctx->pinned;
-        CU(cudaMemcpyAsync(hplan, plan, (max_chunks + 1) * sizeof(int64_t), cudaMemcpyDeviceToHost, st));
-        CU(cudaMemcpyAsync(hplan + max_chunks + 1, offs + nrows, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
-        CU(cudaStreamSynchronize(st));
-        CU(cudaGetLastError());
-        if (hplan[0] < 0) return fail(ctx, FP_ENOMEM, hplan[0] == -2 ? "one row exceeds the list capacity" : "too many list chunks");
-        const int nchunks = (int)hplan[0];
-        std::vector<int64_t> bounds(hplan + 1, hplan + 1 + nchunks);
-        const int64_t total = hplan[max_chunks + 1];
-        // row offsets needed on the host only at chunk boundaries: read them back in one small copy per chunk
-        int64_t r0 = 0;
-        for (int c = 0; c < nchunks; c++) {
-            const int64_t r1 = bounds[c];
-            int64_t base = 0;
-            CU(cudaMemcpyAsync(hplan, offs + r0, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
-            CU(cudaStreamSynchronize(st));
-            base = hplan[0];
-            RowArgs rc = ra; rc.row0 = r0;
-            { ProfScope p(ctx, CAT_FILL, st); launch_fill(order, d, rc, r1 - r0, offs + r0, base, list, st); }
-            CU(cudaGetLastError());
-            { ProfScope p(ctx, CAT_CONTRACT, st);
-              launch_contract(order, d, f, rc, r1 - r0, offs + r0, base, list, pre, partial + r0, st); }
-            CU(cudaGetLastError());
-            r0 = r1;
-        }
-        CU(cudaGetLastError());
+        { ProfScope p(ctx, CAT_RATES, st);
+          CU(launch_rates(order, d, f, ra, nrows, pre, partial, cnt, st)); }
         double *g_out = loc == FP_MEM_DEVICE ? gamma + t0 * nch : o_gamma;
         double *w_out = (loc == FP_MEM_DEVICE && wp) ? wp + t0 * nch : o_wp;
         int64_t *c_out = (loc == FP_MEM_DEVICE && counts) ? counts + t0 * nch : o_cnt;
         { ProfScope p(ctx, CAT_REDUCE, st);
-          launch_finalize(order, d, d_targets, nts, rows_per_unit, partial, cnt, c_over_n, g_out, w_out, c_out, st); }
+          launch_finalize(order, d, nts, rows_per_unit, partial, cnt, c_over_n, g_out, w_out, c_out, st); }
         CU(cudaGetLastError());
         if (loc == FP_MEM_HOST) {
             CU(cudaMemcpyAsync(gamma + t0 * nch, g_out, nts * nch * 8, cudaMemcpyDeviceToHost, st));
             if (wp) CU(cudaMemcpyAsync(wp + t0 * nch, w_out, nts * nch * 8, cudaMemcpyDeviceToHost, st));
             if (counts) CU(cudaMemcpyAsync(counts + t0 * nch, c_out, nts * nch * 8, cudaMemcpyDeviceToHost, st));
         }
-        CU(cudaStreamSynchronize(st));
-        // bookkeeping for the profile (analytic models)
-        ctx->prof.chunks += nchunks;
-        ctx->prof.processes += total;
-        ctx->prof.candidates += nrows * row_cands;
-        ctx->prof.contract_flops += (double)total * (double)f.nblk * 13.0 * 8.0;
+        CU(cudaStreamSynchronize(st));                               // the scratch is reused by the next super-chunk
+        if (ctx->profiling) {                                        // analytic models, DESIGN.md §6
+            std::vector<int64_t> hc(nts * nch);
+            unsigned long long hstat = 0;
+            CU(cudaMemcpy(hc.data(), c_out, nts * nch * 8, cudaMemcpyDeviceToHost));
+            CU(cudaMemcpy(&hstat, stat, 8, cudaMemcpyDeviceToHost));
+            int64_t total = 0;
+            for (int64_t v : hc) total += v;
+            ctx->prof.rows += nrows;
+            ctx->prof.processes += total;
+            ctx->prof.prefiltered += (int64_t)hstat;
+            ctx->prof.candidates += nrows * row_cands;
+            ctx->prof.rates_flops += (double)total * (double)f.nblk * 13.0 * 8.0;
+        }
     }
     return FP_OK;
 }
@@ -524,7 +524,7 @@ static int list_driver(fp_ctx *ctx, int order, int32_t target, int32_t channel, 
     int64_t *offs = sc.take<int64_t>(nrows + 1), *bsums = sc.take<int64_t>(16);
     if (!d_t || !cnt || !offs || !bsums) return fail(ctx, FP_ENOMEM, "scratch");
     CU(cudaMemcpyAsync(d_t, &target, 4, cudaMemcpyHostToDevice, st));
-    RowArgs ra; ra.targets = d_t; ra.row0 = 0; ra.qp_begin = qp; ra.nqp = 1;
+    RowArgs ra; ra.targets = d_t; ra.row0 = 0; ra.qp_begin = qp; ra.nqp = 1; ra.prefiltered = nullptr;
     launch_count(order, d, ra, nrows, cnt, st);
     launch_scan(cnt, nrows, offs, bsums, st);
     std::vector<int64_t> ho(nrows + 1);
@@ -570,18 +570,15 @@ int fp_profile_reset(fp_ctx *ctx) {
 int fp_profile_get(fp_ctx *ctx, fp_profile *out) {
     if (!ctx || !out) return FP_EINVAL;
     fp_profile p = ctx->prof;
-    p.ms_count = p.ms_scan = p.ms_fill = p.ms_precontract = p.ms_contract = p.ms_reduce = 0;
-    p.n_count = p.n_scan = p.n_fill = p.n_precontract = p.n_contract = p.n_reduce = 0;
+    p.ms_precontract = p.ms_rates = p.ms_reduce = 0;
+    p.n_precontract = p.n_rates = p.n_reduce = 0;
     for (auto &e : ctx->events) {
         CU(cudaEventSynchronize(e.b));
         float ms = 0;
         CU(cudaEventElapsedTime(&ms, e.a, e.b));
         switch (e.cat) {
-            case CAT_COUNT: p.ms_count += ms; p.n_count++; break;
-            case CAT_SCAN: p.ms_scan += ms; p.n_scan++; break;
-            case CAT_FILL: p.ms_fill += ms; p.n_fill++; break;
             case CAT_PRE: p.ms_precontract += ms; p.n_precontract++; break;
-            case CAT_CONTRACT: p.ms_contract += ms; p.n_contract++; break;
+            case CAT_RATES: p.ms_rates += ms; p.n_rates++; break;
             case CAT_REDUCE: p.ms_reduce += ms; p.n_reduce++; break;
         }
     }

@@ -26,7 +26,9 @@ struct FpDev {
     int Lmask;                    // L-1 if L is a power of two, else -1
     double B[9];                  // B_mu = b_mu/N_mu, pinned arithmetic
     double scale, ncut, sigma_const, T;
+    float pfK1, pfC2;             // FP32 pre-filter: admit iff Delta_f^2 <= pfK1*|u_a-u_b|_f^2 + pfC2
     const ModeRec *rec;           // N*nb
+    const float4 *recf;           // N*nb  {omega, B1.v, B2.v, B3.v} rounded to FP32; omega = NaN marks a zero mode
     const double *occ;            // N*nb  f_lambda = 1/expm1(hbar omega/kB T)
     const double2 *evec;          // N*nb*nb mass-scaled eigenvectors e~ = e/sqrt(m)
     const double2 *ph1d;          // L
@@ -51,6 +53,7 @@ struct RowArgs {
     const int32_t *targets;       // device
     int64_t row0;                 // first row handled by this launch
     int qp_begin, nqp;            // 4ph only
+    unsigned long long *prefiltered;   // nullable: += candidates admitted by the FP32 pre-filter (profiling)
 };
 
 struct EventRec { int cat; cudaEvent_t a, b; };
@@ -72,26 +75,26 @@ struct fp_ctx {
     size_t pinned_bytes = 0;
 };
 
-enum { CAT_COUNT = 0, CAT_SCAN, CAT_FILL, CAT_PRE, CAT_CONTRACT, CAT_REDUCE };
+enum { CAT_PRE = 0, CAT_RATES, CAT_REDUCE, CAT_N };
 
 // ---- kernel launchers (fp_kernels.cu) --------------------------------------------------------------------------------
 void launch_tables(const FpDev &d, const double *omega, const double *eig, const double *vg, const double *masses_dev,
-                   double hbar_over_kb, ModeRec *rec, double *occ, double2 *evec, double2 *ph1d, int *qc, cudaStream_t st);
-void launch_count(int order, const FpDev &d, const RowArgs &ra, int64_t nrows, uint32_t *counts, cudaStream_t st);
-void launch_scan(const uint32_t *counts, int64_t n, int64_t *offsets /*n+1*/, int64_t *block_sums, cudaStream_t st);
-void launch_plan(const int64_t *offsets, int64_t nrows, int64_t cap, int64_t *plan /*[0]=nchunks, then bounds*/,
-                 int max_chunks, cudaStream_t st);
-void launch_fill(int order, const FpDev &d, const RowArgs &ra, int64_t nrows, const int64_t *offsets, int64_t list_base,
-                 uint32_t *list, cudaStream_t st);
+                   double hbar_over_kb, ModeRec *rec, float4 *recf, double *occ, double2 *evec, double2 *ph1d, int *qc,
+                   unsigned long long *maxima /*2: bits of max omega, max |B v|_2*/, cudaStream_t st);
+// fused rate kernel (fp_rates.cu)
 void launch_pre3(const FpDev &d, const IfcDev &f, const int32_t *targets, int64_t nt, double2 *mhat, cudaStream_t st);
 void launch_pre4(const FpDev &d, const IfcDev &f, const int32_t *targets, int64_t nt, double2 *t0, cudaStream_t st);
-void launch_contract(int order, const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const int64_t *offsets,
-                     int64_t list_base, const uint32_t *list, const double2 *pre, double2 *partial, cudaStream_t st);
-void launch_finalize(int order, const FpDev &d, const int32_t *targets, int64_t nt, int64_t rows_per_unit,
-                     const double2 *partial, const uint32_t *counts, double c_over_n, double *gamma, double *wp,
-                     int64_t *cnt, cudaStream_t st);
+cudaError_t launch_rates(int order, const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const double2 *pre,
+                         double2 *partial, uint32_t *counts, cudaStream_t st);
+size_t rates_smem_bytes(const FpDev &d, const IfcDev &f);
+void launch_finalize(int order, const FpDev &d, int64_t nt, int64_t rows_per_unit, const double2 *partial,
+                     const uint32_t *counts, double c_over_n, double *gamma, double *wp, int64_t *cnt, cudaStream_t st);
 void launch_kappa(const FpDev &d, const double *gamma_total, double pref, double *kappa, cudaStream_t st);
+// process-list export (debug entry points fp_list3 / fp_list4): count -> scan -> ordered fill -> decode
+void launch_count(int order, const FpDev &d, const RowArgs &ra, int64_t nrows, uint32_t *counts, cudaStream_t st);
+void launch_scan(const uint32_t *counts, int64_t n, int64_t *offsets /*n+1*/, int64_t *block_sums, cudaStream_t st);
+void launch_fill(int order, const FpDev &d, const RowArgs &ra, int64_t nrows, const int64_t *offsets, int64_t list_base,
+                 uint32_t *list, cudaStream_t st);
 void launch_decode(int order, const FpDev &d, const RowArgs &ra, const uint32_t *list, int64_t n, int32_t *out,
                    cudaStream_t st);
 double run_fp64_probe(cudaStream_t st, int sm_count);
-size_t contract_smem_bytes(const FpDev &d, const IfcDev &f);

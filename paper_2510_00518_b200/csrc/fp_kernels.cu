@@ -1,149 +1,24 @@
-// fp_kernels.cu -- sm_100a kernels of the FourPhonon hot path.
+// fp_kernels.cu -- sm_100a kernels around the fused rate kernel (fp_rates.cu); SURVEY.md §8(a) rows a1, a4, a8, a9.
 //
-//   k_tables      a1/a4  mode records, BE occupations, mass-scaled eigenvectors, 1-D Bloch phase table
-//   k_count       a2/a3  enumerator count pass: momentum modulo the mesh + energy window
-//                         with the pinned arithmetic of SURVEY.md §8(c) step 3
-//   k_scan_*      a2/a3  exclusive scan of per-row counts -> list offsets (N_accum)
-//   k_fill        a2/a3  fill pass: ordered compaction of allowed candidates into the process list (Algorithm 3,
-//                        PAPER.md:259-316)
-//   k_pre3/k_pre4 a5/a6  per-target pre-contraction of the IFC list with the target eigenvector
-//   k_contract    a5-a7  per-process matrix element |V|^2 (compute_Vp), Gaussian weight and
-//                        occupation factors, block partial sums (Algorithm 4)
-//   k_finalize    a8     fixed-order per-mode reduction, prefactors
+//   k_tables      a1/a4  mode records (FP64 and the FP32 pre-filter copy), BE occupations, mass-scaled
+//                        eigenvectors, 1-D Bloch phase table exp(2 pi i k / L)
+//   k_finalize    a8     fixed-order per-mode reduction of the row partial sums, prefactors
 //   k_kappa       a9     RTA conductivity
-//
-// Contraction algebra: with the momentum modulo, phi(-q_last,R) factorises, so per row
-//   V = sum_b phi(s2 qx, dR_b) sum_{xy} Mhat_b[x][y] A(atomA_b,x) conj(e~_B(atomB_b,y)),
-// where the blocks b=(atomA,atomB,dR) merge all clusters that differ only in legs already fixed by the row, and
-// Mhat_b folds the IFC values with the fixed legs' eigenvectors and phases.  A = e~_A (s2=+) or conj(e~_A) (s2=-).
+//   k_count / k_scan_* / k_fill / k_decode   process-list export for fp_list3 / fp_list4 (Algorithm 3, PAPER.md:259-316:
+//                        count pass, N_accum offsets PAPER.md:265, ordered fill); debug entry points, not on the timed path
+//   k_fp64_probe  DFMA throughput probe (roofline denominator cross-check)
 #include <math_constants.h>
 
-#include "fp_internal.cuh"
+#include "fp_device.cuh"
 
 namespace {
-
-// ---------------------------------------------------------------------------------------------------------------------
-// helpers
-// ---------------------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ double2 cmul(double2 a, double2 b) {
-    return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
-}
-__device__ __forceinline__ void cfma(double2 &acc, double2 a, double2 b) {   // acc += a*b  (4 DFMA)
-    acc.x = fma(a.x, b.x, acc.x);
-    acc.x = fma(-a.y, b.y, acc.x);
-    acc.y = fma(a.x, b.y, acc.y);
-    acc.y = fma(a.y, b.x, acc.y);
-}
-__device__ __forceinline__ int3 unpack_qc(int p) { return make_int3(p & 1023, (p >> 10) & 1023, (p >> 20) & 1023); }
-__device__ __forceinline__ int wrap(int r, int n) {
-    r += (r < 0) ? n : 0;
-    r -= (r >= n) ? n : 0;
-    return r;
-}
-// step 1: component-wise modulo; operands are already in [0,N_mu)
-__device__ __forceinline__ int3 q_add(const FpDev &d, int3 a, int s, int3 b) {
-    return make_int3(wrap(a.x + s * b.x, d.N1), wrap(a.y + s * b.y, d.N2), wrap(a.z + s * b.z, d.N3));
-}
-__device__ __forceinline__ int q_index(const FpDev &d, int3 c) { return c.x + d.N1 * (c.y + d.N2 * c.z); }
-// index into ph1d of phi(q,R): qm = (i1 m1, i2 m2, i3 m3), n = cell offset reduced to [0,N_mu)
-__device__ __forceinline__ int phase_idx(const FpDev &d, int3 qm, int n1, int n2, int n3) {
-    unsigned x = (unsigned)(qm.x * n1 + qm.y * n2 + qm.z * n3);
-    return d.Lmask >= 0 ? (int)(x & (unsigned)d.Lmask) : (int)(x % (unsigned)d.L);
-}
-__device__ __forceinline__ int3 premul(const FpDev &d, int3 c) { return make_int3(c.x * d.m1, c.y * d.m2, c.z * d.m3); }
-
-__device__ __forceinline__ ModeRec load_rec(const ModeRec *p) {
-    const double2 *q = reinterpret_cast<const double2 *>(p);
-    double2 a = __ldg(q), b = __ldg(q + 1);
-    ModeRec r; r.omega = a.x; r.vx = a.y; r.vy = b.x; r.vz = b.y;
-    return r;
-}
-
-struct Row {
-    bool valid;
-    int lam, lam1, s1, s2, ch;
-    int64_t t;
-    int3 qb;          // base q coordinates: q (3ph) or q + s1 q' (4ph)
-    double Obase;     // omega (3ph) or fl(omega + s1 omega') (4ph), pinned
-};
-
-template <int ORDER>
-__device__ __forceinline__ Row make_row(const FpDev &d, const RowArgs &ra, int64_t r) {
-    Row row;
-    if (ORDER == 3) {
-        row.t = r >> 1; row.ch = (int)(r & 1);
-        row.lam = ra.targets[row.t]; row.lam1 = -1;
-        row.s1 = +1; row.s2 = row.ch == 0 ? +1 : -1;
-        double w = d.rec[row.lam].omega;
-        row.valid = (w != 0.0);
-        row.qb = unpack_qc(d.qc[row.lam / d.nb]);
-        row.Obase = w;
-    } else {
-        int j1 = (int)(r % d.nb); r /= d.nb;
-        int qi = (int)(r % ra.nqp); r /= ra.nqp;
-        row.ch = (int)(r % 3); row.t = r / 3;
-        row.lam = ra.targets[row.t];
-        int q1 = ra.qp_begin + qi;
-        row.lam1 = q1 * d.nb + j1;
-        row.s1 = row.ch == 2 ? -1 : +1; row.s2 = row.ch == 0 ? +1 : -1;
-        double w = d.rec[row.lam].omega, w1 = d.rec[row.lam1].omega;
-        row.valid = (w != 0.0) && (w1 != 0.0);
-        row.qb = q_add(d, unpack_qc(d.qc[row.lam / d.nb]), row.s1, unpack_qc(d.qc[q1]));
-        row.Obase = row.s1 > 0 ? __dadd_rn(w, w1) : __dsub_rn(w, w1);
-    }
-    return row;
-}
-
-// compute_sigma(v_A - v_B), in the pinned operation order of SURVEY.md §8(c) step 3 (no FMA contraction)
-__device__ __forceinline__ double sigma_pinned(const FpDev &d, const ModeRec &a, const ModeRec &b) {
-    if (d.sigma_const > 0.0) return d.sigma_const;
-    double dx = __dsub_rn(a.vx, b.vx), dy = __dsub_rn(a.vy, b.vy), dz = __dsub_rn(a.vz, b.vz);
-    double t0 = __dadd_rn(__dadd_rn(__dmul_rn(d.B[0], dx), __dmul_rn(d.B[1], dy)), __dmul_rn(d.B[2], dz));
-    double t1 = __dadd_rn(__dadd_rn(__dmul_rn(d.B[3], dx), __dmul_rn(d.B[4], dy)), __dmul_rn(d.B[5], dz));
-    double t2 = __dadd_rn(__dadd_rn(__dmul_rn(d.B[6], dx), __dmul_rn(d.B[7], dy)), __dmul_rn(d.B[8], dz));
-    double s = __dadd_rn(__dadd_rn(__dmul_rn(t0, t0), __dmul_rn(t1, t1)), __dmul_rn(t2, t2));
-    return __dmul_rn(d.scale, __dsqrt_rn(__ddiv_rn(s, 6.0)));
-}
-
-// Allowed-branch mask of one (qx, ja) pair: bit jb set iff (qx,ja,jb) passes the window (inclusive).
-template <int ORDER>
-__device__ __forceinline__ uint64_t test_pair(const FpDev &d, const Row &row, int p) {
-    ModeRec a = load_rec(d.rec + p);
-    if (a.omega == 0.0) return 0;                                   // item 8: zero modes are never a leg
-    int qx = p / d.nb;
-    int ql = q_index(d, q_add(d, row.qb, row.s2, unpack_qc(d.qc[qx])));
-    const ModeRec *rb = d.rec + (size_t)ql * d.nb;
-    double base = row.s2 > 0 ? __dadd_rn(row.Obase, a.omega) : __dsub_rn(row.Obase, a.omega);
-    uint64_t mask = 0;
-    for (int jb = 0; jb < d.nb; jb++) {
-        ModeRec b = load_rec(rb + jb);
-        if (b.omega == 0.0) continue;
-        double sig = sigma_pinned(d, a, b);
-        double delta = __dsub_rn(base, b.omega);
-        if (sig > 0.0 && fabs(delta) <= __dmul_rn(d.ncut, sig)) mask |= (1ull << jb);
-    }
-    return mask;
-}
-
-// fixed-order block reductions (deterministic: shuffle tree inside a warp, then warp results summed in warp order)
-template <typename T>
-__device__ __forceinline__ T block_sum(T v, T *sh /* >= 32 */) {
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
-    int w = threadIdx.x >> 5, l = threadIdx.x & 31, nw = (blockDim.x + 31) >> 5;
-    __syncthreads();
-    if (l == 0) sh[w] = v;
-    __syncthreads();
-    T tot = 0;
-    if (threadIdx.x == 0)
-        for (int i = 0; i < nw; i++) tot += sh[i];
-    return tot;   // valid in thread 0
-}
 
 // ---------------------------------------------------------------------------------------------------------------------
 // a1 / a4: resident tables
 // ---------------------------------------------------------------------------------------------------------------------
 __global__ void k_tables(FpDev d, const double *omega, const double *eig, const double *vg, const double *masses,
-                         double hbar_over_kb, ModeRec *rec, double *occ, double2 *evec, double2 *ph1d, int *qc) {
+                         double hbar_over_kb, ModeRec *rec, float4 *recf, double *occ, double2 *evec, double2 *ph1d,
+                         int *qc, unsigned long long *maxima) {
     int64_t nmodes = (int64_t)d.N * d.nb;
     int64_t gid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t m = gid; m < nmodes; m += stride) {
@@ -152,6 +27,13 @@ __global__ void k_tables(FpDev d, const double *omega, const double *eig, const 
         rec[m] = r;
         double x = hbar_over_kb * w / d.T;                          // PAPER.md:151  f = 1/(exp(x)-1)
         occ[m] = (w == 0.0) ? 0.0 : 1.0 / expm1(x);
+        // FP32 pre-filter record: u_mu = B_mu . v (so that sigma^2 = scale^2 |u_a - u_b|^2 / 6)
+        double u0 = d.B[0] * r.vx + d.B[1] * r.vy + d.B[2] * r.vz;
+        double u1 = d.B[3] * r.vx + d.B[4] * r.vy + d.B[5] * r.vz;
+        double u2 = d.B[6] * r.vx + d.B[7] * r.vy + d.B[8] * r.vz;
+        recf[m] = make_float4(w == 0.0 ? __int_as_float(0x7fc00000) : (float)w, (float)u0, (float)u1, (float)u2);
+        atomicMax(maxima, (unsigned long long)__double_as_longlong(w));            // non-negative doubles order as integers
+        atomicMax(maxima + 1, (unsigned long long)__double_as_longlong(sqrt(u0 * u0 + u1 * u1 + u2 * u2)));
     }
     int64_t ncomp = nmodes * d.nb;
     for (int64_t c = gid; c < ncomp; c += stride) {
@@ -274,239 +156,6 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_final(const uint32_t *counts, i
     if (blockIdx.x == gridDim.x - 1 && threadIdx.x == 0) offsets[n] = block_sums[gridDim.x];
 }
 
-// chunk planner: greedy maximal runs of rows whose lists fit `cap` entries.  plan[0] = #chunks (or -1), plan[1+k] = end row
-__global__ void k_plan(const int64_t *offsets, int64_t nrows, int64_t cap, int64_t *plan, int max_chunks) {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
-    int64_t r0 = 0;
-    int nch = 0;
-    while (r0 < nrows) {
-        if (nch >= max_chunks) { plan[0] = -1; return; }
-        int64_t lim = offsets[r0] + cap, lo = r0, hi = nrows;        // largest r1 in [r0, nrows] with offsets[r1] <= lim
-        while (lo < hi) {
-            int64_t mid = (lo + hi + 1) >> 1;
-            if (offsets[mid] <= lim) lo = mid; else hi = mid - 1;
-        }
-        if (lo == r0) { plan[0] = -2; return; }                       // a single row exceeds the list capacity
-        plan[1 + nch++] = lo;
-        r0 = lo;
-    }
-    plan[0] = nch;
-}
-
-// ---------------------------------------------------------------------------------------------------------------------
-// a5 / a6 level 0: fold the target eigenvector (and the phase of the last leg at the target q) into the IFC list
-// ---------------------------------------------------------------------------------------------------------------------
-// 3ph: Mhat[t][b][x][y] = sum_{trip in b} conj(phi(q,Rk)) sum_a Phi^{a x y} e~_lam(i,a)          (x: leg j, y: leg k)
-__global__ void __launch_bounds__(256) k_pre3(FpDev d, IfcDev f, const int32_t *targets, double2 *mhat) {
-    int64_t t = blockIdx.x;
-    int lam = targets[t];
-    const double2 *e0 = d.evec + (size_t)lam * d.nb;
-    int3 qm = premul(d, unpack_qc(d.qc[lam / d.nb]));
-    for (int o = threadIdx.x; o < f.nblk * 9; o += blockDim.x) {
-        int b = o / 9, xy = o - 9 * b;
-        double2 acc = make_double2(0.0, 0.0);
-        for (int c = f.blk_start[b]; c < f.blk_start[b + 1]; c++) {
-            int4 m0 = f.cl_meta0[c];
-            double2 ph = d.ph1d[phase_idx(d, qm, m0.y, m0.z, m0.w)];
-            ph.y = -ph.y;                                             // phi(-q, Rk)
-            const double *P = f.phi + (size_t)c * 27 + xy;
-            double2 s = make_double2(0.0, 0.0);
-            for (int a = 0; a < 3; a++) {
-                double2 e = __ldg(e0 + 3 * m0.x + a);
-                double v = P[9 * a];
-                s.x = fma(v, e.x, s.x); s.y = fma(v, e.y, s.y);
-            }
-            cfma(acc, s, ph);
-        }
-        mhat[((size_t)t * f.nblk) * 9 + o] = acc;
-    }
-}
-// 4ph: T0[t][c][b x y] = conj(phi(q,Rl)) sum_a Phi^{a b x y} e~_lam(i,a)
-__global__ void __launch_bounds__(256) k_pre4(FpDev d, IfcDev f, const int32_t *targets, double2 *t0) {
-    int64_t t = blockIdx.x;
-    int lam = targets[t];
-    const double2 *e0 = d.evec + (size_t)lam * d.nb;
-    int3 qm = premul(d, unpack_qc(d.qc[lam / d.nb]));
-    for (int o = threadIdx.x; o < f.n * 27; o += blockDim.x) {
-        int c = o / 27, bxy = o - 27 * c;
-        int4 m0 = f.cl_meta0[c];
-        double2 ph = d.ph1d[phase_idx(d, qm, m0.y, m0.z, m0.w)];
-        ph.y = -ph.y;
-        const double *P = f.phi + (size_t)c * 81 + bxy;
-        double2 s = make_double2(0.0, 0.0);
-        for (int a = 0; a < 3; a++) {
-            double2 e = __ldg(e0 + 3 * m0.x + a);
-            double v = P[27 * a];
-            s.x = fma(v, e.x, s.x); s.y = fma(v, e.y, s.y);
-        }
-        t0[(size_t)t * f.n * 27 + o] = cmul(s, ph);
-    }
-}
-
-// ---------------------------------------------------------------------------------------------------------------------
-// a5 / a6 / a7: contraction + weights
-// ---------------------------------------------------------------------------------------------------------------------
-struct BlkSmem {
-    double2 *M;        // nblk*9   Mhat_b[x][y]
-    int4 *meta;        // nblk     {atomA | atomB<<16, d1, d2, d3}
-    double2 *ph;       // L
-    int *seg;          // nat*nat+1
-};
-
-// One block: u = sum_y (sum_x M[x][y] A[x]) Bc[y];  V += u * phase          (13 complex MAC = 52 DFMA)
-__device__ __forceinline__ void block_term(const double2 *M, const double2 *A, const double2 *Bc, double2 ph, double2 &V) {
-    double2 u = make_double2(0.0, 0.0);
-#pragma unroll
-    for (int y = 0; y < 3; y++) {
-        double2 t = make_double2(0.0, 0.0);
-#pragma unroll
-        for (int x = 0; x < 3; x++) cfma(t, M[3 * x + y], A[x]);
-        cfma(u, t, Bc[y]);
-    }
-    cfma(V, u, ph);
-}
-
-// NAT > 0: eigenvectors of both free legs live in registers, block loop statically split by (atomA, atomB).
-// NAT == 0: generic atom count, eigenvector components are fetched per block (L1/L2-resident table).
-template <int NAT>
-__device__ __forceinline__ double2 contract_process(const FpDev &d, const BlkSmem &bs, int nblk, int lamA, int lamB,
-                                                    int3 qmx, int s2) {
-    double2 V = make_double2(0.0, 0.0);
-    const double2 *eA = d.evec + (size_t)lamA * d.nb, *eB = d.evec + (size_t)lamB * d.nb;
-    if constexpr (NAT > 0) {
-        double2 A[3 * (NAT > 0 ? NAT : 1)], Bc[3 * (NAT > 0 ? NAT : 1)];
-#pragma unroll
-        for (int c = 0; c < 3 * NAT; c++) {
-            A[c] = __ldg(eA + c);
-            if (s2 < 0) A[c].y = -A[c].y;
-            Bc[c] = __ldg(eB + c);
-            Bc[c].y = -Bc[c].y;
-        }
-#pragma unroll
-        for (int a = 0; a < NAT; a++)
-#pragma unroll
-            for (int c = 0; c < NAT; c++) {
-                int b1 = bs.seg[a * NAT + c + 1];
-                for (int b = bs.seg[a * NAT + c]; b < b1; b++) {
-                    int4 m = bs.meta[b];
-                    double2 ph = bs.ph[phase_idx(d, qmx, m.y, m.z, m.w)];
-                    if (s2 < 0) ph.y = -ph.y;
-                    block_term(bs.M + 9 * b, A + 3 * a, Bc + 3 * c, ph, V);
-                }
-            }
-    } else {
-        for (int b = 0; b < nblk; b++) {
-            int4 m = bs.meta[b];
-            int aA = m.x & 0xffff, aB = m.x >> 16;
-            double2 A[3], Bc[3];
-#pragma unroll
-            for (int x = 0; x < 3; x++) {
-                A[x] = __ldg(eA + 3 * aA + x);
-                if (s2 < 0) A[x].y = -A[x].y;
-                Bc[x] = __ldg(eB + 3 * aB + x);
-                Bc[x].y = -Bc[x].y;
-            }
-            double2 ph = bs.ph[phase_idx(d, qmx, m.y, m.z, m.w)];
-            if (s2 < 0) ph.y = -ph.y;
-            block_term(bs.M + 9 * b, A, Bc, ph, V);
-        }
-    }
-    return V;
-}
-
-template <int ORDER, int NAT>
-__global__ void __launch_bounds__(128) k_contract(FpDev d, IfcDev f, RowArgs ra, const int64_t *offsets,
-                                                  int64_t list_base, const uint32_t *list, const double2 *pre,
-                                                  double2 *partial) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ double red[32];
-    int64_t r = blockIdx.x;
-    int64_t beg = offsets[r] - list_base, cnt = offsets[r + 1] - offsets[r];
-    if (cnt == 0) {
-        if (threadIdx.x == 0) partial[r] = make_double2(0.0, 0.0);
-        return;
-    }
-    Row row = make_row<ORDER>(d, ra, ra.row0 + r);
-    BlkSmem bs;                                                      // layout mirrored by contract_smem_bytes()
-    bs.M = reinterpret_cast<double2 *>(smem_raw);
-    bs.ph = bs.M + 9 * f.nblk;
-    double2 *e1 = bs.ph + d.L;                                       // nb entries (level 1 of ORDER 4)
-    bs.meta = reinterpret_cast<int4 *>(e1 + d.nb);
-    bs.seg = reinterpret_cast<int *>(bs.meta + f.nblk);
-
-    for (int i = threadIdx.x; i < d.L; i += blockDim.x) bs.ph[i] = d.ph1d[i];
-    for (int i = threadIdx.x; i < f.nblk; i += blockDim.x) bs.meta[i] = f.blk_meta[i];
-    for (int i = threadIdx.x; i <= d.nat * d.nat; i += blockDim.x) bs.seg[i] = f.seg[i];
-    if (ORDER == 3) {
-        const double2 *src = pre + (size_t)row.t * f.nblk * 9;
-        for (int i = threadIdx.x; i < f.nblk * 9; i += blockDim.x) bs.M[i] = src[i];
-        __syncthreads();
-    } else {
-        // level 1: Mhat_b[x][y] = sum_{c in b} phi(s1 q', Rj-Rl) sum_be T0[c][be][x][y] A'(j_c, be)
-        for (int i = threadIdx.x; i < d.nb; i += blockDim.x) {
-            double2 e = d.evec[(size_t)row.lam1 * d.nb + i];
-            if (row.s1 < 0) e.y = -e.y;
-            e1[i] = e;
-        }
-        __syncthreads();
-        int3 qm1 = premul(d, unpack_qc(d.qc[row.lam1 / d.nb]));
-        const double2 *T0 = pre + (size_t)row.t * f.n * 27;
-        for (int o = threadIdx.x; o < f.nblk * 9; o += blockDim.x) {
-            int b = o / 9, xy = o - 9 * b;
-            double2 acc = make_double2(0.0, 0.0);
-            for (int c = f.blk_start[b]; c < f.blk_start[b + 1]; c++) {
-                int4 m1 = f.cl_meta1[c];
-                double2 ph = bs.ph[phase_idx(d, qm1, m1.y, m1.z, m1.w)];
-                if (row.s1 < 0) ph.y = -ph.y;
-                double2 s = make_double2(0.0, 0.0);
-#pragma unroll
-                for (int be = 0; be < 3; be++) cfma(s, T0[(size_t)c * 27 + 9 * be + xy], e1[3 * m1.x + be]);
-                cfma(acc, s, ph);
-            }
-            bs.M[o] = acc;
-        }
-        __syncthreads();
-    }
-
-    // row-level weight factors
-    const double w0 = d.rec[row.lam].omega;
-    double wrow = w0, f0 = 1.0, occ_row = 1.0;
-    if (ORDER == 4) {
-        double w1 = d.rec[row.lam1].omega, f1 = d.occ[row.lam1];
-        wrow = w0 * w1;
-        f0 = d.occ[row.lam];
-        occ_row = row.s1 > 0 ? 1.0 + f1 : f1;
-    }
-    const double sqrt_pi = 1.7724538509055160273;
-
-    double sG = 0.0, sW = 0.0;
-    for (int64_t i = threadIdx.x; i < cnt; i += blockDim.x) {
-        uint32_t code = list[beg + i];
-        int p = (int)(code / (uint32_t)d.nb), jb = (int)(code - (uint32_t)p * (uint32_t)d.nb);
-        int qx = p / d.nb;
-        int3 xc = unpack_qc(d.qc[qx]);
-        int lamB = q_index(d, q_add(d, row.qb, row.s2, xc)) * d.nb + jb;
-        ModeRec a = load_rec(d.rec + p), b = load_rec(d.rec + lamB);
-        double2 V = contract_process<NAT>(d, bs, f.nblk, p, lamB, premul(d, xc), row.s2);
-        double v2 = V.x * V.x + V.y * V.y;
-        // weights: the same sigma / Delta as the filter, then g = exp(-(Delta/sigma)^2)/(sigma sqrt(pi))
-        double sig = sigma_pinned(d, a, b);
-        double delta = __dsub_rn(row.s2 > 0 ? __dadd_rn(row.Obase, a.omega) : __dsub_rn(row.Obase, a.omega), b.omega);
-        double rr = delta / sig;
-        double g = exp(-(rr * rr)) / (sig * sqrt_pi);
-        double fa = d.occ[p], fb = d.occ[lamB];
-        double occ;
-        if (ORDER == 3) occ = row.s2 > 0 ? (fa - fb) : (fa + fb + 1.0);
-        else occ = occ_row * (row.s2 > 0 ? 1.0 + fa : fa) * fb / f0;
-        double WP = occ * g / (wrow * a.omega * b.omega);
-        sW += WP;
-        sG = fma(WP, v2, sG);
-    }
-    double tG = block_sum<double>(sG, red);
-    double tW = block_sum<double>(sW, red);
-    if (threadIdx.x == 0) partial[r] = make_double2(tG, tW);
-}
-
 // ---------------------------------------------------------------------------------------------------------------------
 // a8: per-mode reduction in fixed order; prefactors C/N^k, symmetry weights
 // ---------------------------------------------------------------------------------------------------------------------
@@ -591,8 +240,10 @@ __global__ void __launch_bounds__(256) k_fp64_probe(int iters, double a, double 
 // launchers
 // ---------------------------------------------------------------------------------------------------------------------
 void launch_tables(const FpDev &d, const double *omega, const double *eig, const double *vg, const double *masses_dev,
-                   double hbar_over_kb, ModeRec *rec, double *occ, double2 *evec, double2 *ph1d, int *qc, cudaStream_t st) {
-    k_tables<<<592, 256, 0, st>>>(d, omega, eig, vg, masses_dev, hbar_over_kb, rec, occ, evec, ph1d, qc);
+                   double hbar_over_kb, ModeRec *rec, float4 *recf, double *occ, double2 *evec, double2 *ph1d, int *qc,
+                   unsigned long long *maxima, cudaStream_t st) {
+    cudaMemsetAsync(maxima, 0, 2 * sizeof(unsigned long long), st);
+    k_tables<<<592, 256, 0, st>>>(d, omega, eig, vg, masses_dev, hbar_over_kb, rec, recf, occ, evec, ph1d, qc, maxima);
 }
 
 void launch_count(int order, const FpDev &d, const RowArgs &ra, int64_t nrows, uint32_t *counts, cudaStream_t st) {
@@ -608,10 +259,6 @@ void launch_scan(const uint32_t *counts, int64_t n, int64_t *offsets, int64_t *b
     k_scan_final<<<(unsigned)nb, SCAN_T, 0, st>>>(counts, n, block_sums, offsets);
 }
 
-void launch_plan(const int64_t *offsets, int64_t nrows, int64_t cap, int64_t *plan, int max_chunks, cudaStream_t st) {
-    k_plan<<<1, 32, 0, st>>>(offsets, nrows, cap, plan, max_chunks);
-}
-
 void launch_fill(int order, const FpDev &d, const RowArgs &ra, int64_t nrows, const int64_t *offsets, int64_t list_base,
                  uint32_t *list, cudaStream_t st) {
     if (nrows <= 0) return;
@@ -619,50 +266,8 @@ void launch_fill(int order, const FpDev &d, const RowArgs &ra, int64_t nrows, co
     else k_fill<4><<<(unsigned)nrows, 256, 0, st>>>(d, ra, offsets, list_base, list);
 }
 
-void launch_pre3(const FpDev &d, const IfcDev &f, const int32_t *targets, int64_t nt, double2 *mhat, cudaStream_t st) {
-    if (nt > 0) k_pre3<<<(unsigned)nt, 256, 0, st>>>(d, f, targets, mhat);
-}
-void launch_pre4(const FpDev &d, const IfcDev &f, const int32_t *targets, int64_t nt, double2 *t0, cudaStream_t st) {
-    if (nt > 0) k_pre4<<<(unsigned)nt, 256, 0, st>>>(d, f, targets, t0);
-}
-
-size_t contract_smem_bytes(const FpDev &d, const IfcDev &f) {
-    size_t b = (size_t)f.nblk * 9 * sizeof(double2) + (size_t)d.L * sizeof(double2) + (size_t)d.nb * sizeof(double2) +
-               (size_t)f.nblk * sizeof(int4) + (size_t)(d.nat * d.nat + 1) * sizeof(int);
-    return (b + 15) & ~(size_t)15;
-}
-
-template <int ORDER, int NAT>
-static void launch_contract_t(const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const int64_t *offsets,
-                              int64_t list_base, const uint32_t *list, const double2 *pre, double2 *partial,
-                              cudaStream_t st) {
-    size_t smem = contract_smem_bytes(d, f);
-    static size_t attr_smem = 0;                                     // opt-in limit is 227 KB minus the static part
-    if (smem > 48 * 1024 && smem > attr_smem) {
-        if (cudaFuncSetAttribute(k_contract<ORDER, NAT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-            return;                                                  // the launch below reports the error
-        attr_smem = smem;
-    }
-    k_contract<ORDER, NAT><<<(unsigned)nrows, 128, smem, st>>>(d, f, ra, offsets, list_base, list, pre, partial);
-}
-
-void launch_contract(int order, const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const int64_t *offsets,
-                     int64_t list_base, const uint32_t *list, const double2 *pre, double2 *partial, cudaStream_t st) {
-    if (nrows <= 0) return;
-#define FP_DISPATCH(O)                                                                                        \
-    switch (d.nat) {                                                                                          \
-        case 1: launch_contract_t<O, 1>(d, f, ra, nrows, offsets, list_base, list, pre, partial, st); break;  \
-        case 2: launch_contract_t<O, 2>(d, f, ra, nrows, offsets, list_base, list, pre, partial, st); break;  \
-        default: launch_contract_t<O, 0>(d, f, ra, nrows, offsets, list_base, list, pre, partial, st); break; \
-    }
-    if (order == 3) { FP_DISPATCH(3) } else { FP_DISPATCH(4) }
-#undef FP_DISPATCH
-}
-
-void launch_finalize(int order, const FpDev &d, const int32_t *targets, int64_t nt, int64_t rows_per_unit,
-                     const double2 *partial, const uint32_t *counts, double c_over_n, double *gamma, double *wp,
-                     int64_t *cnt, cudaStream_t st) {
-    (void)targets;
+void launch_finalize(int order, const FpDev &d, int64_t nt, int64_t rows_per_unit, const double2 *partial,
+                     const uint32_t *counts, double c_over_n, double *gamma, double *wp, int64_t *cnt, cudaStream_t st) {
     if (nt <= 0) return;
     double N = (double)d.N;
     if (order == 3)

@@ -1,0 +1,412 @@
+// fp_rates.cu -- the fused rate kernel of the FourPhonon hot path (SURVEY.md §8(a) rows a2/a3 + a5/a6 + a7) and the
+// per-target pre-contraction.
+//
+//   k_pre3/k_pre4  per-target level-0 contraction of the IFC list with the target eigenvector
+//   k_rates        one CTA per row (3ph: (target, channel); 4ph: (target, channel, lambda')).  Each warp enumerates its
+//                  share of the row's candidates (momentum modulo the mesh PAPER.md:155,288; energy window
+//                  PAPER.md:163,293), compacts the survivors into a warp-private queue in shared memory (ballot-free
+//                  ordered scan), and whenever 32 are queued evaluates them: exact window decision in the pinned FP64
+//                  arithmetic of SURVEY.md §8(c) step 3, matrix element (compute_Vp), Gaussian and
+//                  occupation weights, accumulation.  Nothing is written to global
+//                  memory but one partial sum and one count per row: the process lists of Algorithm 3
+//                   live and die in shared memory.
+//
+// The window is decided twice.  A cheap FP32 pre-filter (table recf: omega and u = B v rounded to FP32) admits a
+// proven superset of the allowed candidates (error budget in DESIGN.md §5.2, constants pfK1/pfC2 from fp_setup); only
+// the ~5 % survivors pay for the pinned FP64 decision, which alone determines counts and rates.
+//
+// Contraction algebra: with the momentum modulo, phi(-q_last,R) factorises, so per row
+//   V = sum_b phi(s2 qx, dR_b) sum_{xy} Mhat_b[x][y] A(atomA_b,x) conj(e~_B(atomB_b,y)),
+// where the blocks b=(atomA,atomB,dR) merge all clusters that differ only in legs already fixed by the row, and
+// Mhat_b folds the IFC values with the fixed legs' eigenvectors and phases.  A = e~_A (s2=+) or conj(e~_A) (s2=-).
+#include "fp_device.cuh"
+
+namespace {
+
+// ---------------------------------------------------------------------------------------------------------------------
+// a5 / a6 level 0: fold the target eigenvector (and the phase of the last leg at the target q) into the IFC list
+// ---------------------------------------------------------------------------------------------------------------------
+// 3ph: Mhat[t][b][x][y] = sum_{trip in b} conj(phi(q,Rk)) sum_a Phi^{a x y} e~_lam(i,a)          (x: leg j, y: leg k)
+__global__ void __launch_bounds__(256) k_pre3(FpDev d, IfcDev f, const int32_t *targets, double2 *mhat) {
+    int64_t t = blockIdx.x;
+    int lam = targets[t];
+    const double2 *e0 = d.evec + (size_t)lam * d.nb;
+    int3 qm = premul(d, unpack_qc(d.qc[lam / d.nb]));
+    for (int o = threadIdx.x; o < f.nblk * 9; o += blockDim.x) {
+        int b = o / 9, xy = o - 9 * b;
+        double2 acc = make_double2(0.0, 0.0);
+        for (int c = f.blk_start[b]; c < f.blk_start[b + 1]; c++) {
+            int4 m0 = f.cl_meta0[c];
+            double2 ph = d.ph1d[phase_idx(d, qm, m0.y, m0.z, m0.w)];
+            ph.y = -ph.y;                                             // phi(-q, Rk)
+            const double *P = f.phi + (size_t)c * 27 + xy;
+            double2 s = make_double2(0.0, 0.0);
+            for (int a = 0; a < 3; a++) {
+                double2 e = __ldg(e0 + 3 * m0.x + a);
+                double v = P[9 * a];
+                s.x = fma(v, e.x, s.x); s.y = fma(v, e.y, s.y);
+            }
+            cfma(acc, s, ph);
+        }
+        mhat[((size_t)t * f.nblk) * 9 + o] = acc;
+    }
+}
+// 4ph: T0[t][c][b x y] = conj(phi(q,Rl)) sum_a Phi^{a b x y} e~_lam(i,a)
+__global__ void __launch_bounds__(256) k_pre4(FpDev d, IfcDev f, const int32_t *targets, double2 *t0) {
+    int64_t t = blockIdx.x;
+    int lam = targets[t];
+    const double2 *e0 = d.evec + (size_t)lam * d.nb;
+    int3 qm = premul(d, unpack_qc(d.qc[lam / d.nb]));
+    for (int o = threadIdx.x; o < f.n * 27; o += blockDim.x) {
+        int c = o / 27, bxy = o - 27 * c;
+        int4 m0 = f.cl_meta0[c];
+        double2 ph = d.ph1d[phase_idx(d, qm, m0.y, m0.z, m0.w)];
+        ph.y = -ph.y;
+        const double *P = f.phi + (size_t)c * 81 + bxy;
+        double2 s = make_double2(0.0, 0.0);
+        for (int a = 0; a < 3; a++) {
+            double2 e = __ldg(e0 + 3 * m0.x + a);
+            double v = P[27 * a];
+            s.x = fma(v, e.x, s.x); s.y = fma(v, e.y, s.y);
+        }
+        t0[(size_t)t * f.n * 27 + o] = cmul(s, ph);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// a5 / a6 / a7: contraction + weights
+// ---------------------------------------------------------------------------------------------------------------------
+struct BlkSmem {
+    double2 *M;        // nblk*9   Mhat_b[x][y]
+    int4 *meta;        // nblk     {atomA | atomB<<16, d1, d2, d3}
+    double2 *ph;       // L
+    int *seg;          // nat*nat+1
+};
+
+// One block: u = sum_y (sum_x M[x][y] A[x]) Bc[y];  V += u * phase          (13 complex MAC = 52 DFMA)
+__device__ __forceinline__ void block_term(const double2 *M, const double2 *A, const double2 *Bc, double2 ph, double2 &V) {
+    double2 u = make_double2(0.0, 0.0);
+#pragma unroll
+    for (int y = 0; y < 3; y++) {
+        double2 t = make_double2(0.0, 0.0);
+#pragma unroll
+        for (int x = 0; x < 3; x++) cfma(t, M[3 * x + y], A[x]);
+        cfma(u, t, Bc[y]);
+    }
+    cfma(V, u, ph);
+}
+
+// NAT > 0: eigenvectors of both free legs live in registers, block loop statically split by (atomA, atomB).
+// NAT == 0: generic atom count, eigenvector components are fetched per block (L1/L2-resident table).
+template <int NAT>
+__device__ __forceinline__ double2 contract_process(const FpDev &d, const BlkSmem &bs, int nblk, int lamA, int lamB,
+                                                    int3 qmx, int s2) {
+    double2 V = make_double2(0.0, 0.0);
+    const double2 *eA = d.evec + (size_t)lamA * d.nb, *eB = d.evec + (size_t)lamB * d.nb;
+    if constexpr (NAT > 0) {
+        double2 A[3 * (NAT > 0 ? NAT : 1)], Bc[3 * (NAT > 0 ? NAT : 1)];
+#pragma unroll
+        for (int c = 0; c < 3 * NAT; c++) {
+            A[c] = __ldg(eA + c);
+            if (s2 < 0) A[c].y = -A[c].y;
+            Bc[c] = __ldg(eB + c);
+            Bc[c].y = -Bc[c].y;
+        }
+#pragma unroll
+        for (int a = 0; a < NAT; a++)
+#pragma unroll
+            for (int c = 0; c < NAT; c++) {
+                int b1 = bs.seg[a * NAT + c + 1];
+                for (int b = bs.seg[a * NAT + c]; b < b1; b++) {
+                    int4 m = bs.meta[b];
+                    double2 ph = bs.ph[phase_idx(d, qmx, m.y, m.z, m.w)];
+                    if (s2 < 0) ph.y = -ph.y;
+                    block_term(bs.M + 9 * b, A + 3 * a, Bc + 3 * c, ph, V);
+                }
+            }
+    } else {
+        const int nat = d.nat;
+        for (int a = 0; a < nat; a++) {                              // blocks are sorted by (atomA, atomB): one
+            double2 A[3];                                            // eigenvector fetch per group, not per block
+#pragma unroll
+            for (int x = 0; x < 3; x++) {
+                A[x] = __ldg(eA + 3 * a + x);
+                if (s2 < 0) A[x].y = -A[x].y;
+            }
+            for (int c = 0; c < nat; c++) {
+                int b0 = bs.seg[a * nat + c], b1 = bs.seg[a * nat + c + 1];
+                if (b0 == b1) continue;
+                double2 Bc[3];
+#pragma unroll
+                for (int x = 0; x < 3; x++) {
+                    Bc[x] = __ldg(eB + 3 * c + x);
+                    Bc[x].y = -Bc[x].y;
+                }
+                for (int b = b0; b < b1; b++) {
+                    int4 m = bs.meta[b];
+                    double2 ph = bs.ph[phase_idx(d, qmx, m.y, m.z, m.w)];
+                    if (s2 < 0) ph.y = -ph.y;
+                    block_term(bs.M + 9 * b, A, Bc, ph, V);
+                }
+            }
+        }
+    }
+    return V;
+}
+
+
+// ---------------------------------------------------------------------------------------------------------------------
+// a2/a3 + a5/a6 + a7: fused enumerate -> shared-memory queue -> evaluate
+// ---------------------------------------------------------------------------------------------------------------------
+constexpr int RT = 128;                       // threads per row CTA
+constexpr int RW = RT / 32;                   // warps
+constexpr int QCAP = 32 + 32 * 36;            // warp queue: < 32 left over + one 6x6 tile of 32 q-points
+
+// Queue entry: qx << 12 | ja << 6 | jb   (N <= 2^20 q-points, nb <= 64)
+__device__ __forceinline__ uint32_t pack_code(int qx, int ja, int jb) { return ((uint32_t)qx << 12) | (ja << 6) | jb; }
+
+struct RowWeights {
+    double wrow;        // omega (3ph) or omega * omega' (4ph)
+    double occ_row;     // 1 (3ph) or (1+f') | f' divided by f (4ph)
+};
+
+template <int ORDER, int NAT>
+__device__ __forceinline__ void eval_process(const FpDev &d, const BlkSmem &bs, int nblk, const Row &row,
+                                             const RowWeights &rw, uint32_t code, bool active, double &sG, double &sW,
+                                             unsigned &cnt) {
+    const int qx = (int)(code >> 12), ja = (int)((code >> 6) & 63u), jb = (int)(code & 63u);
+    const int p = qx * d.nb + ja;
+    const int3 xc = unpack_qc(d.qc[qx]);
+    const int lamB = q_index(d, q_add(d, row.qb, row.s2, xc)) * d.nb + jb;
+    const ModeRec a = load_rec(d.rec + p), b = load_rec(d.rec + lamB);
+    // the decision, in the pinned arithmetic
+    const double sig = sigma_pinned(d, a, b);
+    const double delta = __dsub_rn(row.s2 > 0 ? __dadd_rn(row.Obase, a.omega) : __dsub_rn(row.Obase, a.omega), b.omega);
+    const bool ok = active && a.omega != 0.0 && b.omega != 0.0 && sig > 0.0 && fabs(delta) <= __dmul_rn(d.ncut, sig);
+    if (!__any_sync(0xffffffffu, ok)) return;
+    const double2 V = contract_process<NAT>(d, bs, nblk, p, lamB, premul(d, xc), row.s2);
+    const double v2 = V.x * V.x + V.y * V.y;
+    // weights: g = exp(-(Delta/sigma)^2)/(sigma sqrt(pi)), WP = occ * g / (omega omega' omega'' [omega'''])
+    const double W = rw.wrow * a.omega * b.omega;
+    const double t = 1.0 / (sig * W);
+    const double rr = delta * (t * W);
+    const double g_over_W = exp(-(rr * rr)) * t * 0.56418958354775628695;       // 1/sqrt(pi)
+    const double fa = d.occ[p], fb = d.occ[lamB];
+    double occ;
+    if (ORDER == 3) occ = row.s2 > 0 ? (fa - fb) : (fa + fb + 1.0);
+    else occ = rw.occ_row * (row.s2 > 0 ? 1.0 + fa : fa) * fb;
+    const double WP = occ * g_over_W;
+    if (ok) {
+        sW += WP;
+        sG = fma(WP, v2, sG);
+        cnt++;
+    }
+}
+
+template <int ORDER, int NAT, int TILE>
+__global__ void __launch_bounds__(RT) k_rates(FpDev d, IfcDev f, RowArgs ra, const double2 *pre, double2 *partial,
+                                              uint32_t *counts) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ double red[32];
+    __shared__ unsigned redc[32];
+    __shared__ int tailn[RW];
+    const int64_t r = blockIdx.x;
+    const Row row = make_row<ORDER>(d, ra, ra.row0 + r);
+    if (!row.valid) {                                                 // item 8: zero modes are never a leg
+        if (threadIdx.x == 0) { partial[r] = make_double2(0.0, 0.0); counts[r] = 0; }
+        return;
+    }
+    BlkSmem bs;                                                       // layout mirrored by rates_smem_bytes()
+    bs.M = reinterpret_cast<double2 *>(smem_raw);
+    bs.ph = bs.M + 9 * f.nblk;
+    double2 *e1 = bs.ph + d.L;                                        // nb entries (level 1 of ORDER 4)
+    bs.meta = reinterpret_cast<int4 *>(e1 + d.nb);
+    bs.seg = reinterpret_cast<int *>(bs.meta + f.nblk);
+    uint32_t *queue = reinterpret_cast<uint32_t *>(bs.seg + ((d.nat * d.nat + 1 + 3) & ~3));
+    uint32_t *tailbuf = queue + RW * QCAP;                            // RW*32 entries
+
+    for (int i = threadIdx.x; i < d.L; i += RT) bs.ph[i] = d.ph1d[i];
+    for (int i = threadIdx.x; i < f.nblk; i += RT) bs.meta[i] = f.blk_meta[i];
+    for (int i = threadIdx.x; i <= d.nat * d.nat; i += RT) bs.seg[i] = f.seg[i];
+    if (ORDER == 3) {
+        const double2 *src = pre + (size_t)row.t * f.nblk * 9;
+        for (int i = threadIdx.x; i < f.nblk * 9; i += RT) bs.M[i] = src[i];
+        __syncthreads();
+    } else {
+        // level 1: Mhat_b[x][y] = sum_{c in b} phi(s1 q', Rj-Rl) sum_be T0[c][be][x][y] A'(j_c, be)
+        for (int i = threadIdx.x; i < d.nb; i += RT) {
+            double2 e = d.evec[(size_t)row.lam1 * d.nb + i];
+            if (row.s1 < 0) e.y = -e.y;
+            e1[i] = e;
+        }
+        __syncthreads();
+        const int3 qm1 = premul(d, unpack_qc(d.qc[row.lam1 / d.nb]));
+        const double2 *T0 = pre + (size_t)row.t * f.n * 27;
+        for (int o = threadIdx.x; o < f.nblk * 9; o += RT) {
+            int b = o / 9, xy = o - 9 * b;
+            double2 acc = make_double2(0.0, 0.0);
+            for (int c = f.blk_start[b]; c < f.blk_start[b + 1]; c++) {
+                int4 m1 = f.cl_meta1[c];
+                double2 ph = bs.ph[phase_idx(d, qm1, m1.y, m1.z, m1.w)];
+                if (row.s1 < 0) ph.y = -ph.y;
+                double2 s = make_double2(0.0, 0.0);
+#pragma unroll
+                for (int be = 0; be < 3; be++) cfma(s, T0[(size_t)c * 27 + 9 * be + xy], e1[3 * m1.x + be]);
+                cfma(acc, s, ph);
+            }
+            bs.M[o] = acc;
+        }
+        __syncthreads();
+    }
+
+    RowWeights rw;
+    rw.wrow = d.rec[row.lam].omega;
+    rw.occ_row = 1.0;
+    if (ORDER == 4) {
+        const double f1 = d.occ[row.lam1];
+        rw.wrow *= d.rec[row.lam1].omega;
+        rw.occ_row = (row.s1 > 0 ? 1.0 + f1 : f1) / d.occ[row.lam];
+    }
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint32_t *myq = queue + warp * QCAP;
+    int wq = 0;                                                       // entries queued by this warp (warp-uniform)
+    double sG = 0.0, sW = 0.0;
+    unsigned cnt = 0, nadm = 0;
+
+    // ---- enumerate: FP32 pre-filter over (qx, ja, jb), TILE x TILE branch pairs per q-point in registers -------------
+    const float basef = (float)row.Obase;
+    const float K1 = d.pfK1, C2 = d.pfC2;
+    const float fnan = __int_as_float(0x7fc00000);
+    const int ntile = (d.N + 31) >> 5;
+    for (int tile = warp; tile < ntile; tile += RW) {
+        const int qx = (tile << 5) + lane;
+        const bool inq = qx < d.N;
+        const int qs = inq ? qx : 0;
+        const int ql = q_index(d, q_add(d, row.qb, row.s2, unpack_qc(d.qc[qs])));
+        const float4 *pa = d.recf + (size_t)qs * d.nb, *pb = d.recf + (size_t)ql * d.nb;
+        for (int ja0 = 0; ja0 < d.nb; ja0 += TILE) {
+            float4 A[TILE];
+            float ba[TILE];
+#pragma unroll
+            for (int i = 0; i < TILE; i++) {
+                A[i] = __ldg(pa + ja0 + i);
+                ba[i] = inq ? (row.s2 > 0 ? basef + A[i].x : basef - A[i].x) : fnan;    // omega_f = NaN for zero modes
+            }
+            for (int jb0 = 0; jb0 < d.nb; jb0 += TILE) {
+                uint64_t mask = 0;
+#pragma unroll
+                for (int k = 0; k < TILE; k++) {
+                    const float4 B = __ldg(pb + jb0 + k);
+#pragma unroll
+                    for (int i = 0; i < TILE; i++) {
+                        const float dl = ba[i] - B.x;
+                        const float dx = A[i].y - B.y, dy = A[i].z - B.z, dz = A[i].w - B.w;
+                        const float s = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+                        if (dl * dl <= fmaf(K1, s, C2)) mask |= 1ull << (8 * i + k);
+                    }
+                }
+                // ordered append to the warp queue
+                const unsigned c = __popcll(mask);
+                unsigned incl = c;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    unsigned v = __shfl_up_sync(0xffffffffu, incl, o);
+                    if (lane >= o) incl += v;
+                }
+                const unsigned tot = __shfl_sync(0xffffffffu, incl, 31);
+                if (tot == 0) continue;
+                unsigned pos = wq + incl - c;
+                while (mask) {
+                    const int bit = __ffsll((long long)mask) - 1;
+                    mask &= mask - 1;
+                    myq[pos++] = pack_code(qx, ja0 + (bit >> 3), jb0 + (bit & 7));
+                }
+                wq += tot;
+                nadm += c;
+                __syncwarp();
+                while (wq >= 32) {
+                    wq -= 32;
+                    eval_process<ORDER, NAT>(d, bs, f.nblk, row, rw, myq[wq + lane], true, sG, sW, cnt);
+                }
+                __syncwarp();
+            }
+        }
+    }
+
+    // ---- leftovers of all warps are merged so that at most one batch of the row is partially filled ------------------
+    if (lane == 0) tailn[warp] = wq;
+    __syncthreads();
+    int off = 0, total = 0;
+#pragma unroll
+    for (int w = 0; w < RW; w++) {
+        const int n = tailn[w];
+        if (w < warp) off += n;
+        total += n;
+    }
+    if (lane < wq) tailbuf[off + lane] = myq[lane];
+    __syncthreads();
+    for (int base = warp * 32; base < total; base += RT) {
+        const int idx = base + lane;
+        const bool act = idx < total;
+        eval_process<ORDER, NAT>(d, bs, f.nblk, row, rw, tailbuf[act ? idx : base], act, sG, sW, cnt);
+    }
+
+    const double tG = block_sum<double>(sG, red);
+    const double tW = block_sum<double>(sW, red);
+    const unsigned tC = block_sum<unsigned>(cnt, redc);
+    if (threadIdx.x == 0) { partial[r] = make_double2(tG, tW); counts[r] = tC; }
+    if (ra.prefiltered) {                                             // profiling only: pre-filter survivors
+        const unsigned tA = block_sum<unsigned>(nadm, redc);
+        if (threadIdx.x == 0) atomicAdd(ra.prefiltered, (unsigned long long)tA);
+    }
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------------------------------
+// launchers
+// ---------------------------------------------------------------------------------------------------------------------
+void launch_pre3(const FpDev &d, const IfcDev &f, const int32_t *targets, int64_t nt, double2 *mhat, cudaStream_t st) {
+    if (nt > 0) k_pre3<<<(unsigned)nt, 256, 0, st>>>(d, f, targets, mhat);
+}
+void launch_pre4(const FpDev &d, const IfcDev &f, const int32_t *targets, int64_t nt, double2 *t0, cudaStream_t st) {
+    if (nt > 0) k_pre4<<<(unsigned)nt, 256, 0, st>>>(d, f, targets, t0);
+}
+
+size_t rates_smem_bytes(const FpDev &d, const IfcDev &f) {
+    size_t b = (size_t)f.nblk * 9 * sizeof(double2) + (size_t)d.L * sizeof(double2) + (size_t)d.nb * sizeof(double2) +
+               (size_t)f.nblk * sizeof(int4) + (size_t)((d.nat * d.nat + 1 + 3) & ~3) * sizeof(int) +
+               (size_t)(RW * QCAP + RW * 32) * sizeof(uint32_t);
+    return (b + 15) & ~(size_t)15;
+}
+
+template <int ORDER, int NAT, int TILE>
+static cudaError_t launch_rates_t(const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const double2 *pre,
+                                  double2 *partial, uint32_t *counts, cudaStream_t st) {
+    const size_t smem = rates_smem_bytes(d, f);
+    static size_t attr_smem = 0;                                     // opt-in limit is 227 KB minus the static part
+    if (smem > 48 * 1024 && smem > attr_smem) {
+        cudaError_t e = cudaFuncSetAttribute(k_rates<ORDER, NAT, TILE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        attr_smem = smem;
+    }
+    k_rates<ORDER, NAT, TILE><<<(unsigned)nrows, RT, smem, st>>>(d, f, ra, pre, partial, counts);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_rates(int order, const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const double2 *pre,
+                         double2 *partial, uint32_t *counts, cudaStream_t st) {
+    if (nrows <= 0) return cudaSuccess;
+    const bool t6 = d.nb % 6 == 0;
+#define FP_ARGS d, f, ra, nrows, pre, partial, counts, st
+    if (order == 3) {
+        if (d.nat == 1) return launch_rates_t<3, 1, 3>(FP_ARGS);
+        if (d.nat == 2) return launch_rates_t<3, 2, 6>(FP_ARGS);
+        return t6 ? launch_rates_t<3, 0, 6>(FP_ARGS) : launch_rates_t<3, 0, 3>(FP_ARGS);
+    }
+    if (d.nat == 1) return launch_rates_t<4, 1, 3>(FP_ARGS);
+    if (d.nat == 2) return launch_rates_t<4, 2, 6>(FP_ARGS);
+    return t6 ? launch_rates_t<4, 0, 6>(FP_ARGS) : launch_rates_t<4, 0, 3>(FP_ARGS);
+#undef FP_ARGS
+}

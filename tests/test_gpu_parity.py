@@ -187,16 +187,21 @@ def test_rates4_partial_q_ranges_add_up(fp):
     assert np.all(ge == 0) and np.all(ce == 0)
 
 
-def test_chunked_lists_give_identical_results(fp):
-    """A scratch just above the minimum forces many list chunks (Algorithm 5's mode-by-mode regime)."""
-    inp = fp_inputs.make_config(0)["main"]
-    t = inp.targets3[:96]
+def test_small_scratch_splits_targets_and_gives_identical_results(fp):
+    """A scratch that holds a few targets at a time forces the bounded-memory loop (Algorithm 5)."""
+    inp = fp_inputs.make_tiny("diamond", mesh=(3, 3, 3))
+    t = inp.targets4[6:30]
     with fp.Context.from_inputs(inp, scratch_bytes=64 << 20) as big:
-        g, w, c = big.rates3(t)
-    with fp.Context.from_inputs(inp, scratch_bytes=160 << 10) as small:
+        big.profile_enable(True)
+        g, w, c = big.rates4(t)
+        assert big.profile_get().n_rates == 1
+    with fp.Context.from_inputs(inp, scratch_bytes=512 << 10) as small:
         small.profile_enable(True)
-        gs, ws, cs = small.rates3(t)
-        assert small.profile_get().chunks > 1
+        gs, ws, cs = small.rates4(t)
+        p = small.profile_get()
+        assert p.n_rates > 1
+        assert p.processes == int(cs.sum()) and p.prefiltered >= p.processes
+        assert p.candidates == len(t) * 3 * inp.nq ** 2 * inp.nb ** 3
     assert np.array_equal(c, cs) and np.array_equal(g, gs) and np.array_equal(w, ws)
 
 
@@ -247,8 +252,13 @@ def test_error_codes(fp):
         fp.Context(inp.crystal.lattvec, inp.crystal.masses, inp.omega, inp.eig, inp.vg, inp.mesh,
                    ifc3=(atoms, inp.ifc3[1], inp.ifc3[2]))
     assert e.value.code == fp.FP_EINVAL
-    with pytest.raises(fp.FourPhononError) as e:                           # scratch below one row of candidates
-        with fp.Context.from_inputs(inp, scratch_bytes=1) as ctx:
+    with pytest.raises(fp.FourPhononError) as e:                           # workspace below the resident tables
+        fp.Context.from_inputs(inp, workspace_bytes=4096)
+    assert e.value.code == fp.FP_ENOMEM
+    with fp.Context.from_inputs(inp, scratch_bytes=1) as ctx:             # sized by fp_workspace_bytes: setup fits,
+        need = ctx.workspace.numel()
+    with pytest.raises(fp.FourPhononError) as e:                           # ... but not one target's row arrays
+        with fp.Context.from_inputs(inp, workspace_bytes=need - 60000) as ctx:
             ctx.rates3(inp.targets3[:4])
     assert e.value.code == fp.FP_ENOMEM
 
