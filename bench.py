@@ -266,26 +266,30 @@ def main():
     step_device()
     torch.cuda.synchronize()
     kern = {}
-    flops = procs = cands = launches = 0
+    flops = procs = cands = pref = launches = rows = 0
     for ctx in ctxs:
         p = ctx.profile_get()
-        for k in ("count", "scan", "fill", "precontract", "contract", "reduce"):
+        for k in ("precontract", "rates", "reduce"):
             kern.setdefault(k, [0.0, 0])
             kern[k][0] += getattr(p, "ms_" + k); kern[k][1] += getattr(p, "n_" + k)
-        flops += p.contract_flops; procs += p.processes; cands += p.candidates; launches += p.launches
+        flops += p.rates_flops; procs += p.processes; cands += p.candidates; pref += p.prefiltered
+        launches += p.launches; rows += p.rows
         ctx.profile_enable(False)
     dom = max(kern, key=lambda k: kern[k][0])
-    ms_c, n_c = kern["contract"]
+    ms_c, n_c = kern["rates"]
     achieved = flops / (ms_c * 1e-3) / 1e12 if ms_c > 0 else 0.0
     probe = fp.fp_probe_fp64_tflops()
-    roofline = {"bound": "alu", "kernel": "k_contract (V3/V4 contraction + weights)", "achieved": achieved,
+    roofline = {"bound": "alu", "kernel": "k_rates (fused enumerate + V3/V4 contraction + weights)", "achieved": achieved,
                 "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS, "traffic": None,
-                "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz; DFMA probe on this GPU measured "
-                               f"{probe:.2f} TFLOP/s",
+                "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (MEASURED_PEAKS.json has no FP64 "
+                               f"entry); DFMA probe on this GPU measured {probe:.2f} TFLOP/s",
+                "flops_model": "allowed processes x nblk x 13 complex MAC x 8 flop (DESIGN.md §6); enumeration not counted",
                 "flops_per_launch": flops / max(n_c, 1), "avg_launch_ms": ms_c / max(n_c, 1),
                 "dominant_by_time": dom,
                 "kernel_ms_per_step": {k: round(v[0], 3) for k, v in kern.items()},
-                "candidates_per_step": cands, "processes_per_step": procs}
+                "rows_per_step": rows, "candidates_per_step": cands, "prefiltered_per_step": pref,
+                "processes_per_step": procs,
+                "candidates_per_s_in_k_rates": cands / (ms_c * 1e-3) if ms_c > 0 else 0.0}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
