@@ -132,7 +132,7 @@ size_t ifc_resident_bytes(int64_t n, int order, int nat) {
 
 size_t tables_resident_bytes(int nat, const int32_t mesh[3], long L) {
     size_t N = (size_t)mesh[0] * mesh[1] * mesh[2], nb = 3 * (size_t)nat, M = N * nb;
-    return align_up(M * sizeof(ModeRec)) + align_up(M * 16) + align_up(M * 8) + align_up(M * nb * 16) +
+    return align_up(M * sizeof(ModeRec)) + align_up(M * 16) + align_up(M * 8) * 2 + align_up(M * nb * 16) * 2 +
            align_up((size_t)L * 16) + align_up(N * 4) + align_up(nat * 8) + 256 * 10;
 }
 
@@ -281,16 +281,18 @@ int fp_setup(const fp_crystal *crystal, const double *masses, const double *omeg
     Bump bump{ctx->ws, 0, workspace_bytes};
     ModeRec *rec = bump.take<ModeRec>(M);
     float4 *recf = bump.take<float4>(M);
+    float2 *recn = bump.take<float2>(M);
     unsigned long long *maxima = bump.take<unsigned long long>(2);
     double *occ = bump.take<double>(M);
     double2 *evec = bump.take<double2>(M * nb);
+    double2 *evecc = bump.take<double2>(M * nb);
     double2 *ph1d = bump.take<double2>(L);
     int *qc = bump.take<int>(N);
     double *masses_dev = bump.take<double>(nat);
-    if (!rec || !recf || !maxima || !occ || !evec || !ph1d || !qc || !masses_dev) {
+    if (!rec || !recf || !recn || !maxima || !occ || !evec || !evecc || !ph1d || !qc || !masses_dev) {
         fail(ctx, FP_ENOMEM, "workspace too small for the mode tables"); return bail(FP_ENOMEM);
     }
-    d.rec = rec; d.recf = recf; d.occ = occ; d.evec = evec; d.ph1d = ph1d; d.qc = qc;
+    d.rec = rec; d.recf = recf; d.recn = recn; d.occ = occ; d.evec = evec; d.evecc = evecc; d.ph1d = ph1d; d.qc = qc;
     if (ifc3) { int rc = upload_ifc(ctx, bump, h3, ctx->i3, st); if (rc) return bail(rc); ctx->has3 = true; }
     if (ifc4) { int rc = upload_ifc(ctx, bump, h4, ctx->i4, st); if (rc) return bail(rc); ctx->has4 = true; }
     ctx->resident = align_up(bump.off);
@@ -311,19 +313,24 @@ int fp_setup(const fp_crystal *crystal, const double *masses, const double *omeg
         CU(cudaMemcpyAsync(h_omega.data(), omega, M * 8, cudaMemcpyDeviceToHost, st));
         CU(cudaStreamSynchronize(st));
     }
-    double wmax = 0.0;
+    double wmax = 0.0, wmin = INFINITY;
     for (size_t m = 0; m < M; m++) {
         double w = h_omega[m];
         if (!(w >= 0.0) || !std::isfinite(w)) { fail(ctx, FP_EINVAL, "omega has a NaN, infinite or negative entry"); return bail(FP_EINVAL); }
         wmax = std::max(wmax, w);
+        if (w > 0.0) wmin = std::min(wmin, w);
     }
+    d.wmax = wmax; d.wmin = std::min(wmin, wmax);
     for (size_t m = 0; m < M; m++)
         if (h_omega[m] > 0.0 && h_omega[m] < 1e-6 * wmax) {
             fail(ctx, FP_EINVAL, "omega has a near-zero entry (0 < omega < 1e-6*omega_max); zero modes must be exactly 0");
             return bail(FP_EINVAL);
         }
     CU(cudaMemcpyAsync(masses_dev, masses, nat * 8, cudaMemcpyHostToDevice, st));
-    launch_tables(d, d_omega, d_eig, d_vg, masses_dev, hbar_over_kb(), rec, recf, occ, evec, ph1d, qc, maxima, st);
+    // stage 1 of the FP32 pre-filter: |Delta_f| <= n'_a + n'_b with n' = cs |u| (1+1e-6) + slack
+    d.pfCs = d.sigma_const > 0.0 ? 0.5 * d.ncut * d.sigma_const : d.ncut * d.scale / std::sqrt(6.0);
+    d.pfSlack = 2e-6 * wmax;                                          // per leg; covers |Delta_f - Delta| and 4 FP32 adds
+    launch_tables(d, d_omega, d_eig, d_vg, masses_dev, hbar_over_kb(), rec, recf, recn, occ, evec, evecc, ph1d, qc, maxima, st);
     CU(cudaGetLastError());
     unsigned long long hmax[2] = {0, 0};
     CU(cudaMemcpyAsync(hmax, maxima, sizeof(hmax), cudaMemcpyDeviceToHost, st));
@@ -345,6 +352,9 @@ int fp_setup(const fp_crystal *crystal, const double *masses, const double *omeg
             K1 = cs * cs * (1.0 + eta + 1e-5); C2 = dd * dd * (1.0 + 1.0 / eta) * (1.0 + 1e-5);
         }
         if (!(K1 < 1e30) || !(C2 < 1e30)) { K1 = 0.0; C2 = INFINITY; }  // filter disabled (ncut = inf): admit everything
+        // upper bound of every entry of the stage 1 table (same formula as k_tables, rounded up once more)
+        const double nmax = (d.sigma_const > 0.0 ? d.pfCs : d.pfCs * umax) * (1.0 + 2e-6) + d.pfSlack;
+        d.pfNmax = std::isfinite(nmax) ? std::nextafterf((float)nmax, INFINITY) : INFINITY;
         d.pfK1 = std::nextafterf((float)K1, INFINITY);
         d.pfC2 = std::isinf(C2) ? INFINITY : std::nextafterf((float)C2, INFINITY);
     }

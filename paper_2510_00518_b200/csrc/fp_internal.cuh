@@ -26,11 +26,16 @@ struct FpDev {
     int Lmask;                    // L-1 if L is a power of two, else -1
     double B[9];                  // B_mu = b_mu/N_mu, pinned arithmetic
     double scale, ncut, sigma_const, T;
-    float pfK1, pfC2;             // FP32 pre-filter: admit iff Delta_f^2 <= pfK1*|u_a-u_b|_f^2 + pfC2
+    float pfK1, pfC2;             // FP32 pre-filter, stage 2: admit iff Delta_f^2 <= pfK1*|u_a-u_b|_f^2 + pfC2
+    double pfCs, pfSlack;         // stage 1 table constants: n' = cs*|u|*(1+1e-6) + slack (k_tables)
+    float pfNmax;                 // max n' over all modes; wmin/wmax: range of the non-zero frequencies (row_is_empty)
+    double wmin, wmax;
     const ModeRec *rec;           // N*nb
     const float4 *recf;           // N*nb  {omega, B1.v, B2.v, B3.v} rounded to FP32; omega = NaN marks a zero mode
+    const float2 *recn;           // N*nb  {omega (NaN for zero modes), n'} stage 1: admit iff |Delta_f| <= n'_a + n'_b
     const double *occ;            // N*nb  f_lambda = 1/expm1(hbar omega/kB T)
     const double2 *evec;          // N*nb*nb mass-scaled eigenvectors e~ = e/sqrt(m)
+    const double2 *evecc;         // N*nb*nb conj(e~): the conjugations of step 6 are table choices, not arithmetic
     const double2 *ph1d;          // L
     const int *qc;                // N packed mesh coordinates i1 | i2<<10 | i3<<20   (N_mu <= 1024)
 };
@@ -79,7 +84,7 @@ enum { CAT_PRE = 0, CAT_RATES, CAT_REDUCE, CAT_N };
 
 // ---- kernel launchers (fp_kernels.cu) --------------------------------------------------------------------------------
 void launch_tables(const FpDev &d, const double *omega, const double *eig, const double *vg, const double *masses_dev,
-                   double hbar_over_kb, ModeRec *rec, float4 *recf, double *occ, double2 *evec, double2 *ph1d, int *qc,
+                   double hbar_over_kb, ModeRec *rec, float4 *recf, float2 *recn, double *occ, double2 *evec, double2 *evecc, double2 *ph1d, int *qc,
                    unsigned long long *maxima /*2: bits of max omega, max |B v|_2*/, cudaStream_t st);
 // fused rate kernel (fp_rates.cu)
 void launch_pre3(const FpDev &d, const IfcDev &f, const int32_t *targets, int64_t nt, double2 *mhat, cudaStream_t st);

@@ -17,7 +17,7 @@ namespace {
 // a1 / a4: resident tables
 // ---------------------------------------------------------------------------------------------------------------------
 __global__ void k_tables(FpDev d, const double *omega, const double *eig, const double *vg, const double *masses,
-                         double hbar_over_kb, ModeRec *rec, float4 *recf, double *occ, double2 *evec, double2 *ph1d,
+                         double hbar_over_kb, ModeRec *rec, float4 *recf, float2 *recn, double *occ, double2 *evec, double2 *evecc, double2 *ph1d,
                          int *qc, unsigned long long *maxima) {
     int64_t nmodes = (int64_t)d.N * d.nb;
     int64_t gid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, stride = (int64_t)gridDim.x * blockDim.x;
@@ -31,15 +31,22 @@ __global__ void k_tables(FpDev d, const double *omega, const double *eig, const 
         double u0 = d.B[0] * r.vx + d.B[1] * r.vy + d.B[2] * r.vz;
         double u1 = d.B[3] * r.vx + d.B[4] * r.vy + d.B[5] * r.vz;
         double u2 = d.B[6] * r.vx + d.B[7] * r.vy + d.B[8] * r.vz;
-        recf[m] = make_float4(w == 0.0 ? __int_as_float(0x7fc00000) : (float)w, (float)u0, (float)u1, (float)u2);
+        const float wf = w == 0.0 ? __int_as_float(0x7fc00000) : (float)w;
+        recf[m] = make_float4(wf, (float)u0, (float)u1, (float)u2);
+        // stage 1 record: n' >= cs |u| + slack, rounded up (cs = ncut scale/sqrt(6), or n' = ncut sigma_const/2 + slack)
+        const double un = sqrt(u0 * u0 + u1 * u1 + u2 * u2);
+        const double nn = (d.sigma_const > 0.0 ? d.pfCs : d.pfCs * un) * (1.0 + 1e-6) + d.pfSlack;
+        recn[m] = make_float2(wf, isinf(d.pfCs) ? CUDART_INF_F : __double2float_ru(nn));   // ncut = inf: admit everything
         atomicMax(maxima, (unsigned long long)__double_as_longlong(w));            // non-negative doubles order as integers
-        atomicMax(maxima + 1, (unsigned long long)__double_as_longlong(sqrt(u0 * u0 + u1 * u1 + u2 * u2)));
+        atomicMax(maxima + 1, (unsigned long long)__double_as_longlong(un));
     }
     int64_t ncomp = nmodes * d.nb;
     for (int64_t c = gid; c < ncomp; c += stride) {
         int atom = (int)(c % d.nb) / 3;
         double sm = sqrt(masses[atom]);
-        evec[c] = make_double2(eig[2 * c] / sm, eig[2 * c + 1] / sm);
+        const double2 e = make_double2(eig[2 * c] / sm, eig[2 * c + 1] / sm);
+        evec[c] = e;
+        evecc[c] = make_double2(e.x, -e.y);
     }
     for (int64_t k = gid; k < d.L; k += stride) {                   // a4: phi = exp(2 pi i k / L)
         double s, c;
@@ -240,10 +247,10 @@ __global__ void __launch_bounds__(256) k_fp64_probe(int iters, double a, double 
 // launchers
 // ---------------------------------------------------------------------------------------------------------------------
 void launch_tables(const FpDev &d, const double *omega, const double *eig, const double *vg, const double *masses_dev,
-                   double hbar_over_kb, ModeRec *rec, float4 *recf, double *occ, double2 *evec, double2 *ph1d, int *qc,
+                   double hbar_over_kb, ModeRec *rec, float4 *recf, float2 *recn, double *occ, double2 *evec, double2 *evecc, double2 *ph1d, int *qc,
                    unsigned long long *maxima, cudaStream_t st) {
     cudaMemsetAsync(maxima, 0, 2 * sizeof(unsigned long long), st);
-    k_tables<<<592, 256, 0, st>>>(d, omega, eig, vg, masses_dev, hbar_over_kb, rec, recf, occ, evec, ph1d, qc, maxima);
+    k_tables<<<592, 256, 0, st>>>(d, omega, eig, vg, masses_dev, hbar_over_kb, rec, recf, recn, occ, evec, evecc, ph1d, qc, maxima);
 }
 
 void launch_count(int order, const FpDev &d, const RowArgs &ra, int64_t nrows, uint32_t *counts, cudaStream_t st) {

@@ -98,30 +98,24 @@ __device__ __forceinline__ void block_term(const double2 *M, const double2 *A, c
 
 // NAT > 0: eigenvectors of both free legs live in registers, block loop statically split by (atomA, atomB).
 // NAT == 0: generic atom count, eigenvector components are fetched per block (L1/L2-resident table).
+// eA points at e~_A (s2=+) or conj(e~_A) (s2=-), eB at conj(e~_B); bs.ph holds phi (s2=+) or conj(phi) (s2=-): the
+// conjugations of step 6 are table choices made once per row, not arithmetic in the loop.
 template <int NAT>
-__device__ __forceinline__ double2 contract_process(const FpDev &d, const BlkSmem &bs, int nblk, int lamA, int lamB,
-                                                    int3 qmx, int s2) {
+__device__ __forceinline__ double2 contract_process(const FpDev &d, const BlkSmem &bs, const double2 *__restrict__ eA,
+                                                    const double2 *__restrict__ eB, int3 qmx) {
     double2 V = make_double2(0.0, 0.0);
-    const double2 *eA = d.evec + (size_t)lamA * d.nb, *eB = d.evec + (size_t)lamB * d.nb;
     if constexpr (NAT > 0) {
         double2 A[3 * (NAT > 0 ? NAT : 1)], Bc[3 * (NAT > 0 ? NAT : 1)];
 #pragma unroll
-        for (int c = 0; c < 3 * NAT; c++) {
-            A[c] = __ldg(eA + c);
-            if (s2 < 0) A[c].y = -A[c].y;
-            Bc[c] = __ldg(eB + c);
-            Bc[c].y = -Bc[c].y;
-        }
+        for (int c = 0; c < 3 * NAT; c++) { A[c] = __ldg(eA + c); Bc[c] = __ldg(eB + c); }
 #pragma unroll
         for (int a = 0; a < NAT; a++)
 #pragma unroll
             for (int c = 0; c < NAT; c++) {
-                int b1 = bs.seg[a * NAT + c + 1];
+                const int b1 = bs.seg[a * NAT + c + 1];
                 for (int b = bs.seg[a * NAT + c]; b < b1; b++) {
-                    int4 m = bs.meta[b];
-                    double2 ph = bs.ph[phase_idx(d, qmx, m.y, m.z, m.w)];
-                    if (s2 < 0) ph.y = -ph.y;
-                    block_term(bs.M + 9 * b, A + 3 * a, Bc + 3 * c, ph, V);
+                    const int4 m = bs.meta[b];
+                    block_term(bs.M + 9 * b, A + 3 * a, Bc + 3 * c, bs.ph[phase_idx(d, qmx, m.y, m.z, m.w)], V);
                 }
             }
     } else {
@@ -129,24 +123,16 @@ __device__ __forceinline__ double2 contract_process(const FpDev &d, const BlkSme
         for (int a = 0; a < nat; a++) {                              // blocks are sorted by (atomA, atomB): one
             double2 A[3];                                            // eigenvector fetch per group, not per block
 #pragma unroll
-            for (int x = 0; x < 3; x++) {
-                A[x] = __ldg(eA + 3 * a + x);
-                if (s2 < 0) A[x].y = -A[x].y;
-            }
+            for (int x = 0; x < 3; x++) A[x] = __ldg(eA + 3 * a + x);
             for (int c = 0; c < nat; c++) {
-                int b0 = bs.seg[a * nat + c], b1 = bs.seg[a * nat + c + 1];
+                const int b0 = bs.seg[a * nat + c], b1 = bs.seg[a * nat + c + 1];
                 if (b0 == b1) continue;
                 double2 Bc[3];
 #pragma unroll
-                for (int x = 0; x < 3; x++) {
-                    Bc[x] = __ldg(eB + 3 * c + x);
-                    Bc[x].y = -Bc[x].y;
-                }
+                for (int x = 0; x < 3; x++) Bc[x] = __ldg(eB + 3 * c + x);
                 for (int b = b0; b < b1; b++) {
-                    int4 m = bs.meta[b];
-                    double2 ph = bs.ph[phase_idx(d, qmx, m.y, m.z, m.w)];
-                    if (s2 < 0) ph.y = -ph.y;
-                    block_term(bs.M + 9 * b, A, Bc, ph, V);
+                    const int4 m = bs.meta[b];
+                    block_term(bs.M + 9 * b, A, Bc, bs.ph[phase_idx(d, qmx, m.y, m.z, m.w)], V);
                 }
             }
         }
@@ -160,7 +146,8 @@ __device__ __forceinline__ double2 contract_process(const FpDev &d, const BlkSme
 // ---------------------------------------------------------------------------------------------------------------------
 constexpr int RT = 128;                       // threads per row CTA
 constexpr int RW = RT / 32;                   // warps
-constexpr int QCAP = 32 + 32 * 36;            // warp queue: < 32 left over + one 6x6 tile of 32 q-points
+constexpr int PCAP = 32 + 32 * 36;            // pending queue: < 32 left over + one 6x6 sub-tile of 32 q-points
+constexpr int QCAP = 64;                      // evaluation queue: < 32 left over + one stage-2 round
 
 // Queue entry: qx << 12 | ja << 6 | jb   (N <= 2^20 q-points, nb <= 64)
 __device__ __forceinline__ uint32_t pack_code(int qx, int ja, int jb) { return ((uint32_t)qx << 12) | (ja << 6) | jb; }
@@ -171,7 +158,7 @@ struct RowWeights {
 };
 
 template <int ORDER, int NAT>
-__device__ __forceinline__ void eval_process(const FpDev &d, const BlkSmem &bs, int nblk, const Row &row,
+__device__ __forceinline__ void eval_process(const FpDev &d, const BlkSmem &bs, const Row &row,
                                              const RowWeights &rw, uint32_t code, bool active, double &sG, double &sW,
                                              unsigned &cnt) {
     const int qx = (int)(code >> 12), ja = (int)((code >> 6) & 63u), jb = (int)(code & 63u);
@@ -184,7 +171,8 @@ __device__ __forceinline__ void eval_process(const FpDev &d, const BlkSmem &bs, 
     const double delta = __dsub_rn(row.s2 > 0 ? __dadd_rn(row.Obase, a.omega) : __dsub_rn(row.Obase, a.omega), b.omega);
     const bool ok = active && a.omega != 0.0 && b.omega != 0.0 && sig > 0.0 && fabs(delta) <= __dmul_rn(d.ncut, sig);
     if (!__any_sync(0xffffffffu, ok)) return;
-    const double2 V = contract_process<NAT>(d, bs, nblk, p, lamB, premul(d, xc), row.s2);
+    const double2 V = contract_process<NAT>(d, bs, (row.s2 > 0 ? d.evec : d.evecc) + (size_t)p * d.nb,
+                                            d.evecc + (size_t)lamB * d.nb, premul(d, xc));
     const double v2 = V.x * V.x + V.y * V.y;
     // weights: g = exp(-(Delta/sigma)^2)/(sigma sqrt(pi)), WP = occ * g / (omega omega' omega'' [omega'''])
     const double W = rw.wrow * a.omega * b.omega;
@@ -203,16 +191,36 @@ __device__ __forceinline__ void eval_process(const FpDev &d, const BlkSmem &bs, 
     }
 }
 
+// FP32 pre-filter, stage 2, of one candidate code (table recf): Delta_f^2 <= K1 |u_a - u_b|_f^2 + C2
+__device__ __forceinline__ bool prefilter2(const FpDev &d, const Row &row, float basef, uint32_t code) {
+    const int qx = (int)(code >> 12), ja = (int)((code >> 6) & 63u), jb = (int)(code & 63u);
+    const int ql = q_index(d, q_add(d, row.qb, row.s2, unpack_qc(d.qc[qx])));
+    const float4 A = __ldg(d.recf + (size_t)qx * d.nb + ja), B = __ldg(d.recf + (size_t)ql * d.nb + jb);
+    const float dl = (row.s2 > 0 ? basef + A.x : basef - A.x) - B.x;
+    const float dx = A.y - B.y, dy = A.z - B.z, dz = A.w - B.w;
+    const float s = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    return dl * dl <= fmaf(d.pfK1, s, d.pfC2);
+}
+
+// No candidate of the row can pass the window: |Delta| <= ncut sigma <= n_a + n_b <= 2 nmax for every allowed process,
+// and Delta = base + s2 omega_A - omega_B with both legs' frequencies in [wmin, wmax] (the non-zero modes).
+__device__ __forceinline__ bool row_is_empty(const FpDev &d, const Row &row) {
+    const double w2 = 2.0 * (double)d.pfNmax, lo = d.wmin, hi = d.wmax;
+    const double dmin = row.s2 > 0 ? row.Obase + lo - hi : row.Obase - 2.0 * hi;
+    const double dmax = row.s2 > 0 ? row.Obase + hi - lo : row.Obase - 2.0 * lo;
+    return dmin > w2 || dmax < -w2;
+}
+
 template <int ORDER, int NAT, int TILE>
-__global__ void __launch_bounds__(RT) k_rates(FpDev d, IfcDev f, RowArgs ra, const double2 *pre, double2 *partial,
-                                              uint32_t *counts) {
+__global__ void __launch_bounds__(RT, 4) k_rates(FpDev d, IfcDev f, RowArgs ra, const double2 *pre, double2 *partial,
+                                                 uint32_t *counts) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ double red[32];
     __shared__ unsigned redc[32];
     __shared__ int tailn[RW];
     const int64_t r = blockIdx.x;
     const Row row = make_row<ORDER>(d, ra, ra.row0 + r);
-    if (!row.valid) {                                                 // item 8: zero modes are never a leg
+    if (!row.valid || row_is_empty(d, row)) {                         // item 8: zero modes are never a leg
         if (threadIdx.x == 0) { partial[r] = make_double2(0.0, 0.0); counts[r] = 0; }
         return;
     }
@@ -223,22 +231,22 @@ __global__ void __launch_bounds__(RT) k_rates(FpDev d, IfcDev f, RowArgs ra, con
     bs.meta = reinterpret_cast<int4 *>(e1 + d.nb);
     bs.seg = reinterpret_cast<int *>(bs.meta + f.nblk);
     uint32_t *queue = reinterpret_cast<uint32_t *>(bs.seg + ((d.nat * d.nat + 1 + 3) & ~3));
-    uint32_t *tailbuf = queue + RW * QCAP;                            // RW*32 entries
+    uint32_t *tailbuf = queue + RW * (PCAP + QCAP);                   // RW*32 entries
 
-    for (int i = threadIdx.x; i < d.L; i += RT) bs.ph[i] = d.ph1d[i];
     for (int i = threadIdx.x; i < f.nblk; i += RT) bs.meta[i] = f.blk_meta[i];
     for (int i = threadIdx.x; i <= d.nat * d.nat; i += RT) bs.seg[i] = f.seg[i];
     if (ORDER == 3) {
         const double2 *src = pre + (size_t)row.t * f.nblk * 9;
         for (int i = threadIdx.x; i < f.nblk * 9; i += RT) bs.M[i] = src[i];
-        __syncthreads();
     } else {
         // level 1: Mhat_b[x][y] = sum_{c in b} phi(s1 q', Rj-Rl) sum_be T0[c][be][x][y] A'(j_c, be)
-        for (int i = threadIdx.x; i < d.nb; i += RT) {
-            double2 e = d.evec[(size_t)row.lam1 * d.nb + i];
-            if (row.s1 < 0) e.y = -e.y;
-            e1[i] = e;
+        for (int i = threadIdx.x; i < d.L; i += RT) {
+            double2 p = d.ph1d[i];
+            if (row.s1 < 0) p.y = -p.y;
+            bs.ph[i] = p;
         }
+        const double2 *ev1 = (row.s1 > 0 ? d.evec : d.evecc) + (size_t)row.lam1 * d.nb;
+        for (int i = threadIdx.x; i < d.nb; i += RT) e1[i] = ev1[i];
         __syncthreads();
         const int3 qm1 = premul(d, unpack_qc(d.qc[row.lam1 / d.nb]));
         const double2 *T0 = pre + (size_t)row.t * f.n * 27;
@@ -248,7 +256,6 @@ __global__ void __launch_bounds__(RT) k_rates(FpDev d, IfcDev f, RowArgs ra, con
             for (int c = f.blk_start[b]; c < f.blk_start[b + 1]; c++) {
                 int4 m1 = f.cl_meta1[c];
                 double2 ph = bs.ph[phase_idx(d, qm1, m1.y, m1.z, m1.w)];
-                if (row.s1 < 0) ph.y = -ph.y;
                 double2 s = make_double2(0.0, 0.0);
 #pragma unroll
                 for (int be = 0; be < 3; be++) cfma(s, T0[(size_t)c * 27 + 9 * be + xy], e1[3 * m1.x + be]);
@@ -258,6 +265,12 @@ __global__ void __launch_bounds__(RT) k_rates(FpDev d, IfcDev f, RowArgs ra, con
         }
         __syncthreads();
     }
+    for (int i = threadIdx.x; i < d.L; i += RT) {                     // phases of the free legs: phi(s2 qx, dR)
+        double2 p = d.ph1d[i];
+        if (row.s2 < 0) p.y = -p.y;
+        bs.ph[i] = p;
+    }
+    __syncthreads();
 
     RowWeights rw;
     rw.wrow = d.rec[row.lam].omega;
@@ -269,87 +282,108 @@ __global__ void __launch_bounds__(RT) k_rates(FpDev d, IfcDev f, RowArgs ra, con
     }
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    uint32_t *myq = queue + warp * QCAP;
-    int wq = 0;                                                       // entries queued by this warp (warp-uniform)
+    uint32_t *pend = queue + warp * (PCAP + QCAP);                    // stage-1 survivors of this warp
+    uint32_t *myq = pend + PCAP;                                      // stage-2 survivors, evaluated 32 at a time
+    int wp = 0, wq = 0;                                               // entries in pend / myq (warp-uniform)
     double sG = 0.0, sW = 0.0;
     unsigned cnt = 0, nadm = 0;
 
-    // ---- enumerate: FP32 pre-filter over (qx, ja, jb), TILE x TILE branch pairs per q-point in registers -------------
+    // ---- one loop, one evaluation site: evaluate a full batch if one is queued, else refill the queue -------------------
+    //   enumerate a sub-tile (32 q-points x TILE x TILE branch pairs) with the FP32 pre-filter, two stages:
+    //     stage 1 (2 compares per pair, table recn):          |Delta_f| <= n'_a + n'_b   (sigma <= cs(|u_a| + |u_b|))
+    //     stage 2 (warp-cooperative on the survivors, recf):  Delta_f^2 <= K1 |u_a - u_b|_f^2 + C2
+    //   Both admit every candidate the pinned FP64 decision allows, which alone decides.
     const float basef = (float)row.Obase;
-    const float K1 = d.pfK1, C2 = d.pfC2;
     const float fnan = __int_as_float(0x7fc00000);
     const int ntile = (d.N + 31) >> 5;
-    for (int tile = warp; tile < ntile; tile += RW) {
-        const int qx = (tile << 5) + lane;
-        const bool inq = qx < d.N;
-        const int qs = inq ? qx : 0;
-        const int ql = q_index(d, q_add(d, row.qb, row.s2, unpack_qc(d.qc[qs])));
-        const float4 *pa = d.recf + (size_t)qs * d.nb, *pb = d.recf + (size_t)ql * d.nb;
-        for (int ja0 = 0; ja0 < d.nb; ja0 += TILE) {
-            float4 A[TILE];
-            float ba[TILE];
+    constexpr bool ONE_SUB = (NAT > 0 && 3 * NAT == TILE);            // nb == TILE: one sub-tile per q-tile
+    const int nsub = ONE_SUB ? 1 : d.nb / TILE;
+    const int nsteps = ntile * nsub * nsub;
+    int step = warp, phase = 0, tbase = 0, total = 0;                 // phase 0 enumerate, 1 flush pend, 2 merged tails
+    for (;;) {
+        __syncwarp();
+        uint32_t code = 0;
+        bool act = false, have = false;
+        if (wq >= 32) {
+            wq -= 32; code = myq[wq + lane]; act = true; have = true;
+        } else if (phase == 2) {
+            if (tbase >= total) break;
+            const int idx = tbase + lane;
+            act = idx < total; code = tailbuf[act ? idx : tbase]; tbase += RT; have = true;
+        }
+        if (have) {
+            eval_process<ORDER, NAT>(d, bs, row, rw, code, act, sG, sW, cnt);
+            continue;
+        }
+        if (wp >= 32 || (phase == 1 && wp > 0)) {                     // stage 2 on up to 32 pending candidates
+            const int n = wp < 32 ? wp : 32;
+            wp -= n;
+            const bool in = lane < n;
+            const uint32_t c2 = pend[wp + (in ? lane : 0)];
+            const bool pass = in && prefilter2(d, row, basef, c2);
+            const unsigned bal = __ballot_sync(0xffffffffu, pass);
+            if (pass) myq[wq + __popc(bal & ((1u << lane) - 1u))] = c2;
+            wq += __popc(bal);
+            nadm += pass ? 1u : 0u;
+            continue;
+        }
+        if (phase == 0) {
+            if (step >= nsteps) { phase = 1; continue; }
+            const int tile = ONE_SUB ? step : step / (nsub * nsub), sub = ONE_SUB ? 0 : step - tile * nsub * nsub;
+            const int ja0 = ONE_SUB ? 0 : (sub / nsub) * TILE, jb0 = ONE_SUB ? 0 : (sub - (sub / nsub) * nsub) * TILE;
+            step += RW;
+            const int qx = (tile << 5) + lane;
+            const bool inq = qx < d.N;
+            const int qs = inq ? qx : 0;
+            const int ql = q_index(d, q_add(d, row.qb, row.s2, unpack_qc(d.qc[qs])));
+            const float2 *pa = d.recn + (size_t)qs * d.nb + ja0, *pb = d.recn + (size_t)ql * d.nb + jb0;
+            float lo[TILE], hi[TILE];
 #pragma unroll
             for (int i = 0; i < TILE; i++) {
-                A[i] = __ldg(pa + ja0 + i);
-                ba[i] = inq ? (row.s2 > 0 ? basef + A[i].x : basef - A[i].x) : fnan;    // omega_f = NaN for zero modes
+                const float2 A = __ldg(pa + i);                       // omega_f = NaN for zero modes: never admitted
+                const float ba = inq ? (row.s2 > 0 ? basef + A.x : basef - A.x) : fnan;
+                lo[i] = ba - A.y; hi[i] = ba + A.y;
             }
-            for (int jb0 = 0; jb0 < d.nb; jb0 += TILE) {
-                uint64_t mask = 0;
+            uint64_t mask = 0;
 #pragma unroll
-                for (int k = 0; k < TILE; k++) {
-                    const float4 B = __ldg(pb + jb0 + k);
+            for (int k = 0; k < TILE; k++) {
+                const float2 B = __ldg(pb + k);
+                const float bl = B.x - B.y, bh = B.x + B.y;
 #pragma unroll
-                    for (int i = 0; i < TILE; i++) {
-                        const float dl = ba[i] - B.x;
-                        const float dx = A[i].y - B.y, dy = A[i].z - B.z, dz = A[i].w - B.w;
-                        const float s = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-                        if (dl * dl <= fmaf(K1, s, C2)) mask |= 1ull << (8 * i + k);
-                    }
-                }
-                // ordered append to the warp queue
-                const unsigned c = __popcll(mask);
-                unsigned incl = c;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    unsigned v = __shfl_up_sync(0xffffffffu, incl, o);
-                    if (lane >= o) incl += v;
-                }
-                const unsigned tot = __shfl_sync(0xffffffffu, incl, 31);
-                if (tot == 0) continue;
-                unsigned pos = wq + incl - c;
-                while (mask) {
-                    const int bit = __ffsll((long long)mask) - 1;
-                    mask &= mask - 1;
-                    myq[pos++] = pack_code(qx, ja0 + (bit >> 3), jb0 + (bit & 7));
-                }
-                wq += tot;
-                nadm += c;
-                __syncwarp();
-                while (wq >= 32) {
-                    wq -= 32;
-                    eval_process<ORDER, NAT>(d, bs, f.nblk, row, rw, myq[wq + lane], true, sG, sW, cnt);
-                }
-                __syncwarp();
+                for (int i = 0; i < TILE; i++)
+                    if (bl <= hi[i] && bh >= lo[i]) mask |= 1ull << (8 * i + k);
             }
+            // ordered append to the pending queue
+            const unsigned c = __popcll(mask);
+            unsigned incl = c;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                unsigned v = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += v;
+            }
+            unsigned pos = wp + incl - c;
+            while (mask) {
+                const int bit = __ffsll((long long)mask) - 1;
+                mask &= mask - 1;
+                pend[pos++] = pack_code(qx, ja0 + (bit >> 3), jb0 + (bit & 7));
+            }
+            wp += __shfl_sync(0xffffffffu, incl, 31);
+            continue;
         }
-    }
-
-    // ---- leftovers of all warps are merged so that at most one batch of the row is partially filled ------------------
-    if (lane == 0) tailn[warp] = wq;
-    __syncthreads();
-    int off = 0, total = 0;
+        // phase 1 with pend empty and fewer than 32 queued: merge the leftovers of all warps so that at most one batch
+        // of the row is partially filled
+        if (lane == 0) tailn[warp] = wq;
+        __syncthreads();
+        int off = 0;
 #pragma unroll
-    for (int w = 0; w < RW; w++) {
-        const int n = tailn[w];
-        if (w < warp) off += n;
-        total += n;
-    }
-    if (lane < wq) tailbuf[off + lane] = myq[lane];
-    __syncthreads();
-    for (int base = warp * 32; base < total; base += RT) {
-        const int idx = base + lane;
-        const bool act = idx < total;
-        eval_process<ORDER, NAT>(d, bs, f.nblk, row, rw, tailbuf[act ? idx : base], act, sG, sW, cnt);
+        for (int w = 0; w < RW; w++) {
+            const int n = tailn[w];
+            if (w < warp) off += n;
+            total += n;
+        }
+        if (lane < wq) tailbuf[off + lane] = myq[lane];
+        __syncthreads();
+        wq = 0; phase = 2; tbase = warp * 32;
     }
 
     const double tG = block_sum<double>(sG, red);
@@ -377,7 +411,7 @@ void launch_pre4(const FpDev &d, const IfcDev &f, const int32_t *targets, int64_
 size_t rates_smem_bytes(const FpDev &d, const IfcDev &f) {
     size_t b = (size_t)f.nblk * 9 * sizeof(double2) + (size_t)d.L * sizeof(double2) + (size_t)d.nb * sizeof(double2) +
                (size_t)f.nblk * sizeof(int4) + (size_t)((d.nat * d.nat + 1 + 3) & ~3) * sizeof(int) +
-               (size_t)(RW * QCAP + RW * 32) * sizeof(uint32_t);
+               (size_t)(RW * (PCAP + QCAP) + RW * 32) * sizeof(uint32_t);
     return (b + 15) & ~(size_t)15;
 }
 
