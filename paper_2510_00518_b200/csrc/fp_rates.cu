@@ -102,12 +102,10 @@ __device__ __forceinline__ void block_term(const double2 *M, const double2 *A, c
 // conjugations of step 6 are table choices made once per row, not arithmetic in the loop.
 template <int NAT>
 __device__ __forceinline__ double2 contract_process(const FpDev &d, const BlkSmem &bs, const double2 *__restrict__ eA,
-                                                    const double2 *__restrict__ eB, int3 qmx) {
+                                                    const double2 *__restrict__ eB, const double2 *A, const double2 *Bc,
+                                                    int3 qmx) {
     double2 V = make_double2(0.0, 0.0);
-    if constexpr (NAT > 0) {
-        double2 A[3 * (NAT > 0 ? NAT : 1)], Bc[3 * (NAT > 0 ? NAT : 1)];
-#pragma unroll
-        for (int c = 0; c < 3 * NAT; c++) { A[c] = __ldg(eA + c); Bc[c] = __ldg(eB + c); }
+    if constexpr (NAT > 0) {                                         // A, Bc: registers, loaded by the caller
 #pragma unroll
         for (int a = 0; a < NAT; a++)
 #pragma unroll
@@ -121,18 +119,18 @@ __device__ __forceinline__ double2 contract_process(const FpDev &d, const BlkSme
     } else {
         const int nat = d.nat;
         for (int a = 0; a < nat; a++) {                              // blocks are sorted by (atomA, atomB): one
-            double2 A[3];                                            // eigenvector fetch per group, not per block
+            double2 Ag[3];                                           // eigenvector fetch per group, not per block
 #pragma unroll
-            for (int x = 0; x < 3; x++) A[x] = __ldg(eA + 3 * a + x);
+            for (int x = 0; x < 3; x++) Ag[x] = __ldg(eA + 3 * a + x);
             for (int c = 0; c < nat; c++) {
                 const int b0 = bs.seg[a * nat + c], b1 = bs.seg[a * nat + c + 1];
                 if (b0 == b1) continue;
-                double2 Bc[3];
+                double2 Bg[3];
 #pragma unroll
-                for (int x = 0; x < 3; x++) Bc[x] = __ldg(eB + 3 * c + x);
+                for (int x = 0; x < 3; x++) Bg[x] = __ldg(eB + 3 * c + x);
                 for (int b = b0; b < b1; b++) {
                     const int4 m = bs.meta[b];
-                    block_term(bs.M + 9 * b, A, Bc, bs.ph[phase_idx(d, qmx, m.y, m.z, m.w)], V);
+                    block_term(bs.M + 9 * b, Ag, Bg, bs.ph[phase_idx(d, qmx, m.y, m.z, m.w)], V);
                 }
             }
         }
@@ -144,12 +142,20 @@ __device__ __forceinline__ double2 contract_process(const FpDev &d, const BlkSme
 // ---------------------------------------------------------------------------------------------------------------------
 // a2/a3 + a5/a6 + a7: fused enumerate -> shared-memory queue -> evaluate
 // ---------------------------------------------------------------------------------------------------------------------
+#ifndef FP_MINB
+#define FP_MINB 4                             // resident CTAs per SM the register allocation targets
+#endif
+#ifndef FP_PREFETCH
+#define FP_PREFETCH 0                         // stage 2 prefetches the records and eigenvectors of its survivors into L1
+#endif
 constexpr int RT = 128;                       // threads per row CTA
 constexpr int RW = RT / 32;                   // warps
 constexpr int PCAP = 32 + 32 * 36;            // pending queue: < 32 left over + one 6x6 sub-tile of 32 q-points
 constexpr int QCAP = 64;                      // evaluation queue: < 32 left over + one stage-2 round
 
-// Queue entry: qx << 12 | ja << 6 | jb   (N <= 2^20 q-points, nb <= 64)
+// Evaluation-queue entry: {qA << 6 | jA, qB << 6 | jB}: both legs are addressable at once, so every load of a batch
+// is issued before the first dependent instruction.
+// Pending-queue entry: qx << 12 | ja << 6 | jb   (N <= 2^20 q-points, nb <= 64)
 __device__ __forceinline__ uint32_t pack_code(int qx, int ja, int jb) { return ((uint32_t)qx << 12) | (ja << 6) | jb; }
 
 struct RowWeights {
@@ -159,27 +165,32 @@ struct RowWeights {
 
 template <int ORDER, int NAT>
 __device__ __forceinline__ void eval_process(const FpDev &d, const BlkSmem &bs, const Row &row,
-                                             const RowWeights &rw, uint32_t code, bool active, double &sG, double &sW,
+                                             const RowWeights &rw, uint2 ent, bool active, double &sG, double &sW,
                                              unsigned &cnt) {
-    const int qx = (int)(code >> 12), ja = (int)((code >> 6) & 63u), jb = (int)(code & 63u);
-    const int p = qx * d.nb + ja;
-    const int3 xc = unpack_qc(d.qc[qx]);
-    const int lamB = q_index(d, q_add(d, row.qb, row.s2, xc)) * d.nb + jb;
+    const int qx = (int)(ent.x >> 6);
+    const int p = qx * d.nb + (int)(ent.x & 63u), lamB = (int)(ent.y >> 6) * d.nb + (int)(ent.y & 63u);
+    // all loads of the batch up front: mode records, occupations, mesh coordinates, both eigenvectors
+    const double2 *eA = (row.s2 > 0 ? d.evec : d.evecc) + (size_t)p * d.nb, *eB = d.evecc + (size_t)lamB * d.nb;
     const ModeRec a = load_rec(d.rec + p), b = load_rec(d.rec + lamB);
+    const double fa = __ldg(d.occ + p), fb = __ldg(d.occ + lamB);
+    const int3 xc = unpack_qc(__ldg(d.qc + qx));
+    double2 A[3 * (NAT > 0 ? NAT : 1)], Bc[3 * (NAT > 0 ? NAT : 1)];
+    if constexpr (NAT > 0) {
+#pragma unroll
+        for (int c = 0; c < 3 * NAT; c++) { A[c] = __ldg(eA + c); Bc[c] = __ldg(eB + c); }
+    }
     // the decision, in the pinned arithmetic
     const double sig = sigma_pinned(d, a, b);
     const double delta = __dsub_rn(row.s2 > 0 ? __dadd_rn(row.Obase, a.omega) : __dsub_rn(row.Obase, a.omega), b.omega);
     const bool ok = active && a.omega != 0.0 && b.omega != 0.0 && sig > 0.0 && fabs(delta) <= __dmul_rn(d.ncut, sig);
     if (!__any_sync(0xffffffffu, ok)) return;
-    const double2 V = contract_process<NAT>(d, bs, (row.s2 > 0 ? d.evec : d.evecc) + (size_t)p * d.nb,
-                                            d.evecc + (size_t)lamB * d.nb, premul(d, xc));
+    const double2 V = contract_process<NAT>(d, bs, eA, eB, A, Bc, premul(d, xc));
     const double v2 = V.x * V.x + V.y * V.y;
     // weights: g = exp(-(Delta/sigma)^2)/(sigma sqrt(pi)), WP = occ * g / (omega omega' omega'' [omega'''])
     const double W = rw.wrow * a.omega * b.omega;
     const double t = 1.0 / (sig * W);
     const double rr = delta * (t * W);
     const double g_over_W = exp(-(rr * rr)) * t * 0.56418958354775628695;       // 1/sqrt(pi)
-    const double fa = d.occ[p], fb = d.occ[lamB];
     double occ;
     if (ORDER == 3) occ = row.s2 > 0 ? (fa - fb) : (fa + fb + 1.0);
     else occ = rw.occ_row * (row.s2 > 0 ? 1.0 + fa : fa) * fb;
@@ -191,15 +202,31 @@ __device__ __forceinline__ void eval_process(const FpDev &d, const BlkSmem &bs, 
     }
 }
 
+#if FP_PREFETCH
+__device__ __forceinline__ void prefetch_l1(const void *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+#endif
+
 // FP32 pre-filter, stage 2, of one candidate code (table recf): Delta_f^2 <= K1 |u_a - u_b|_f^2 + C2
-__device__ __forceinline__ bool prefilter2(const FpDev &d, const Row &row, float basef, uint32_t code) {
+__device__ __forceinline__ bool prefilter2(const FpDev &d, const Row &row, float basef, uint32_t code, uint2 &ent) {
     const int qx = (int)(code >> 12), ja = (int)((code >> 6) & 63u), jb = (int)(code & 63u);
-    const int ql = q_index(d, q_add(d, row.qb, row.s2, unpack_qc(d.qc[qx])));
+    const int ql = q_index(d, q_add(d, row.qb, row.s2, unpack_qc(__ldg(d.qc + qx))));
+    ent = make_uint2(((uint32_t)qx << 6) | (uint32_t)ja, ((uint32_t)ql << 6) | (uint32_t)jb);   // evaluation-queue entry
     const float4 A = __ldg(d.recf + (size_t)qx * d.nb + ja), B = __ldg(d.recf + (size_t)ql * d.nb + jb);
     const float dl = (row.s2 > 0 ? basef + A.x : basef - A.x) - B.x;
     const float dx = A.y - B.y, dy = A.z - B.z, dz = A.w - B.w;
     const float s = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-    return dl * dl <= fmaf(d.pfK1, s, d.pfC2);
+    const bool pass = dl * dl <= fmaf(d.pfK1, s, d.pfC2);
+#if FP_PREFETCH
+    if (pass) {
+        const size_t pa = (size_t)qx * d.nb + ja, pb = (size_t)ql * d.nb + jb;
+        const char *ea = reinterpret_cast<const char *>((row.s2 > 0 ? d.evec : d.evecc) + pa * d.nb);
+        const char *eb = reinterpret_cast<const char *>(d.evecc + pb * d.nb);
+        const int last = d.nb * 16 - 16;
+        prefetch_l1(d.rec + pa); prefetch_l1(d.rec + pb);
+        prefetch_l1(ea); prefetch_l1(ea + last); prefetch_l1(eb); prefetch_l1(eb + last);
+    }
+#endif
+    return pass;
 }
 
 // No candidate of the row can pass the window: |Delta| <= ncut sigma <= n_a + n_b <= 2 nmax for every allowed process,
@@ -212,7 +239,7 @@ __device__ __forceinline__ bool row_is_empty(const FpDev &d, const Row &row) {
 }
 
 template <int ORDER, int NAT, int TILE>
-__global__ void __launch_bounds__(RT, 4) k_rates(FpDev d, IfcDev f, RowArgs ra, const double2 *pre, double2 *partial,
+__global__ void __launch_bounds__(RT, FP_MINB) k_rates(FpDev d, IfcDev f, RowArgs ra, const double2 *pre, double2 *partial,
                                                  uint32_t *counts) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ double red[32];
@@ -230,8 +257,9 @@ __global__ void __launch_bounds__(RT, 4) k_rates(FpDev d, IfcDev f, RowArgs ra, 
     double2 *e1 = bs.ph + d.L;                                        // nb entries (level 1 of ORDER 4)
     bs.meta = reinterpret_cast<int4 *>(e1 + d.nb);
     bs.seg = reinterpret_cast<int *>(bs.meta + f.nblk);
-    uint32_t *queue = reinterpret_cast<uint32_t *>(bs.seg + ((d.nat * d.nat + 1 + 3) & ~3));
-    uint32_t *tailbuf = queue + RW * (PCAP + QCAP);                   // RW*32 entries
+    uint2 *evq = reinterpret_cast<uint2 *>(bs.seg + ((d.nat * d.nat + 1 + 3) & ~3));   // RW*QCAP, then RW*32 (tails)
+    uint2 *tailbuf = evq + RW * QCAP;
+    uint32_t *pendq = reinterpret_cast<uint32_t *>(tailbuf + RW * 32);                // RW*PCAP
 
     for (int i = threadIdx.x; i < f.nblk; i += RT) bs.meta[i] = f.blk_meta[i];
     for (int i = threadIdx.x; i <= d.nat * d.nat; i += RT) bs.seg[i] = f.seg[i];
@@ -282,8 +310,8 @@ __global__ void __launch_bounds__(RT, 4) k_rates(FpDev d, IfcDev f, RowArgs ra, 
     }
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    uint32_t *pend = queue + warp * (PCAP + QCAP);                    // stage-1 survivors of this warp
-    uint32_t *myq = pend + PCAP;                                      // stage-2 survivors, evaluated 32 at a time
+    uint32_t *pend = pendq + warp * PCAP;                             // stage-1 survivors of this warp
+    uint2 *myq = evq + warp * QCAP;                                   // stage-2 survivors, evaluated 32 at a time
     int wp = 0, wq = 0;                                               // entries in pend / myq (warp-uniform)
     double sG = 0.0, sW = 0.0;
     unsigned cnt = 0, nadm = 0;
@@ -302,17 +330,17 @@ __global__ void __launch_bounds__(RT, 4) k_rates(FpDev d, IfcDev f, RowArgs ra, 
     int step = warp, phase = 0, tbase = 0, total = 0;                 // phase 0 enumerate, 1 flush pend, 2 merged tails
     for (;;) {
         __syncwarp();
-        uint32_t code = 0;
+        uint2 ent = make_uint2(0u, 0u);
         bool act = false, have = false;
         if (wq >= 32) {
-            wq -= 32; code = myq[wq + lane]; act = true; have = true;
+            wq -= 32; ent = myq[wq + lane]; act = true; have = true;
         } else if (phase == 2) {
             if (tbase >= total) break;
             const int idx = tbase + lane;
-            act = idx < total; code = tailbuf[act ? idx : tbase]; tbase += RT; have = true;
+            act = idx < total; ent = tailbuf[act ? idx : tbase]; tbase += RT; have = true;
         }
         if (have) {
-            eval_process<ORDER, NAT>(d, bs, row, rw, code, act, sG, sW, cnt);
+            eval_process<ORDER, NAT>(d, bs, row, rw, ent, act, sG, sW, cnt);
             continue;
         }
         if (wp >= 32 || (phase == 1 && wp > 0)) {                     // stage 2 on up to 32 pending candidates
@@ -320,9 +348,10 @@ __global__ void __launch_bounds__(RT, 4) k_rates(FpDev d, IfcDev f, RowArgs ra, 
             wp -= n;
             const bool in = lane < n;
             const uint32_t c2 = pend[wp + (in ? lane : 0)];
-            const bool pass = in && prefilter2(d, row, basef, c2);
+            uint2 e2;
+            const bool pass = prefilter2(d, row, basef, c2, e2) && in;
             const unsigned bal = __ballot_sync(0xffffffffu, pass);
-            if (pass) myq[wq + __popc(bal & ((1u << lane) - 1u))] = c2;
+            if (pass) myq[wq + __popc(bal & ((1u << lane) - 1u))] = e2;
             wq += __popc(bal);
             nadm += pass ? 1u : 0u;
             continue;
@@ -411,7 +440,7 @@ void launch_pre4(const FpDev &d, const IfcDev &f, const int32_t *targets, int64_
 size_t rates_smem_bytes(const FpDev &d, const IfcDev &f) {
     size_t b = (size_t)f.nblk * 9 * sizeof(double2) + (size_t)d.L * sizeof(double2) + (size_t)d.nb * sizeof(double2) +
                (size_t)f.nblk * sizeof(int4) + (size_t)((d.nat * d.nat + 1 + 3) & ~3) * sizeof(int) +
-               (size_t)(RW * (PCAP + QCAP) + RW * 32) * sizeof(uint32_t);
+               (size_t)(RW * QCAP + RW * 32) * sizeof(uint2) + (size_t)(RW * PCAP) * sizeof(uint32_t);
     return (b + 15) & ~(size_t)15;
 }
 
