@@ -153,6 +153,8 @@ def main():
     ap.add_argument("--impl", default="b200")
     ap.add_argument("--scratch-gb", type=float, default=16.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--path", choices=["auto", "fused", "split", "split-serial"], default="auto",
+                    help="execution path of fp_rates3/4 (fp_set_path); auto = split when the scratch holds the lists")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -174,9 +176,12 @@ def main():
 
     jobs = workload(args.config)
     scratch = int(args.scratch_gb * (1 << 30))
+    path_id = {"auto": fp.FP_PATH_AUTO, "fused": fp.FP_PATH_FUSED, "split": fp.FP_PATH_SPLIT,
+               "split-serial": fp.FP_PATH_SPLIT_SERIAL}[args.path]
     ctxs, dev_targets = [], []
     for inp, t3, t4 in jobs:
         ctx = fp.Context.from_inputs(inp, scratch_bytes=scratch, device=dev)
+        ctx.set_path(path_id)
         ctxs.append(ctx)
         dev_targets.append((None if t3 is None else torch.from_numpy(np.ascontiguousarray(t3)).to(dev),
                             None if t4 is None else torch.from_numpy(np.ascontiguousarray(t4)).to(dev)))
@@ -202,6 +207,7 @@ def main():
         res = {}
         for inp, t3, t4 in jobs:
             with fp.Context.from_inputs(inp, scratch_bytes=scratch, device=dev) as ctx:
+                ctx.set_path(path_id)
                 h2d += inp.omega.nbytes + inp.eig.nbytes + inp.vg.nbytes
                 for ifc in (inp.ifc3, inp.ifc4):
                     if ifc is not None:
@@ -269,7 +275,7 @@ def main():
     flops = procs = cands = pref = launches = rows = 0
     for ctx in ctxs:
         p = ctx.profile_get()
-        for k in ("precontract", "rates", "reduce"):
+        for k in ("precontract", "enum", "rates", "reduce"):
             kern.setdefault(k, [0.0, 0])
             kern[k][0] += getattr(p, "ms_" + k); kern[k][1] += getattr(p, "n_" + k)
         flops += p.rates_flops; procs += p.processes; cands += p.candidates; pref += p.prefiltered

@@ -84,6 +84,8 @@ typedef struct {
     int64_t prefiltered;    /* candidates admitted by the FP32 pre-filter (superset of the allowed ones)            */
     int64_t processes;      /* allowed processes (pinned FP64 decision) evaluated                                   */
     double  rates_flops;    /* FP64 flops of the per-process contraction (analytic model)             */
+    double  ms_enum;        /* split path: summed durations of the enumerator kernel (ms_rates is then the evaluator) */
+    int64_t n_enum;
 } fp_profile;
 
 /* Bytes of workspace fp_setup needs for its resident tables plus `scratch_bytes` of per-call scratch (per-target
@@ -134,6 +136,17 @@ int fp_list3(fp_ctx *ctx, int32_t target, int32_t channel, int32_t *pairs, int64
  *   triples HOST cap*3 int32.                                                                                        */
 int fp_list4(fp_ctx *ctx, int32_t target, int32_t channel, int32_t qp, int32_t *triples, int64_t cap, int64_t *n,
              void *stream);
+
+/* Execution path of fp_rates3 / fp_rates4 (same results bit for bit in counts, within rounding order in rates):
+ *   FP_PATH_SPLIT  enumerator kernel -> process lists in the scratch region -> evaluator kernel (Algorithms 3 and 4,
+ *                  PAPER.md:259-352, both on the device), chunks of rows sized to the scratch;
+ *   FP_PATH_FUSED  one kernel per chunk of targets, lists in shared memory only (needs 20 bytes of scratch per row);
+ *   FP_PATH_AUTO   (default) split when the scratch holds the lists of at least a few hundred rows, else fused.     */
+#define FP_PATH_AUTO  0
+#define FP_PATH_FUSED 1
+#define FP_PATH_SPLIT 2
+#define FP_PATH_SPLIT_SERIAL 3   /* split without the two-stream overlap of enumerator and evaluator (for measurement) */
+int fp_set_path(fp_ctx *ctx, int path);
 
 /* Profiling of the library's own kernels (off by default; adds two cudaEventRecord per launch).                     */
 int fp_profile_enable(fp_ctx *ctx, int on);

@@ -17,6 +17,7 @@ from pathlib import Path
 import numpy as np
 
 FP_OK, FP_EINVAL, FP_ENOMEM, FP_ECUDA, FP_ESTATE = 0, -1, -2, -3, -4
+FP_PATH_AUTO, FP_PATH_FUSED, FP_PATH_SPLIT, FP_PATH_SPLIT_SERIAL = 0, 1, 2, 3
 FP_MEM_HOST, FP_MEM_DEVICE = 0, 1
 
 _PKG = Path(__file__).resolve().parent
@@ -27,7 +28,7 @@ _SOURCES = ["fp_kernels.cu", "fp_rates.cu", "fp_host.cu"]
 # every symbol include/fourphonon.h declares (tests check that the built library exports all of them)
 EXPORTED_SYMBOLS = [
     "fp_workspace_bytes", "fp_setup", "fp_rates3", "fp_rates4", "fp_kappa_rta", "fp_list3", "fp_list4",
-    "fp_profile_enable", "fp_profile_reset", "fp_profile_get", "fp_probe_fp64_tflops", "fp_constants",
+    "fp_set_path", "fp_profile_enable", "fp_profile_reset", "fp_profile_get", "fp_probe_fp64_tflops", "fp_constants",
     "fp_last_error", "fp_version", "fp_destroy",
 ]
 
@@ -72,7 +73,8 @@ class _Broadening(C.Structure):
 class _Profile(C.Structure):
     _fields_ = [(n, C.c_double) for n in ("ms_precontract", "ms_rates", "ms_reduce")] + \
                [(n, C.c_int64) for n in ("n_precontract", "n_rates", "n_reduce", "rows", "candidates", "prefiltered",
-                                         "processes")] + [("rates_flops", C.c_double)]
+                                         "processes")] + [("rates_flops", C.c_double), ("ms_enum", C.c_double),
+                                                          ("n_enum", C.c_int64)]
 
 
 @dataclass
@@ -88,10 +90,12 @@ class Profile:
     prefiltered: int
     processes: int
     rates_flops: float
+    ms_enum: float = 0.0
+    n_enum: int = 0
 
     @property
     def launches(self) -> int:
-        return self.n_precontract + self.n_rates + self.n_reduce
+        return self.n_precontract + self.n_rates + self.n_reduce + self.n_enum
 
 
 _lib = None
@@ -121,6 +125,8 @@ def load_library():
     lib.fp_list3.argtypes = [vp, i32, i32, vp, i64, C.POINTER(i64), vp]
     lib.fp_list4.restype = C.c_int
     lib.fp_list4.argtypes = [vp, i32, i32, i32, vp, i64, C.POINTER(i64), vp]
+    lib.fp_set_path.restype = C.c_int
+    lib.fp_set_path.argtypes = [vp, C.c_int]
     lib.fp_profile_enable.restype = C.c_int
     lib.fp_profile_enable.argtypes = [vp, C.c_int]
     lib.fp_profile_reset.restype = C.c_int
@@ -356,6 +362,10 @@ class Context:
             self._check(self.lib.fp_list4(self.ctx, int(target), int(channel), int(qp), out.ctypes.data, n.value,
                                           C.byref(n), _stream_ptr(stream)))
         return out[:n.value]
+
+    def set_path(self, path: int):
+        """FP_PATH_AUTO / FP_PATH_FUSED / FP_PATH_SPLIT / FP_PATH_SPLIT_SERIAL (include/fourphonon.h)."""
+        self._check(self.lib.fp_set_path(self.ctx, int(path)))
 
     def profile_enable(self, on=True):
         self._check(self.lib.fp_profile_enable(self.ctx, 1 if on else 0))

@@ -63,7 +63,7 @@ long gcdl(long a, long b) { while (b) { long t = a % b; a = b; b = t; } return a
 
 // Host-side analysis of an IFC list: group clusters into contraction blocks (atomA, atomB, dR) -- DESIGN.md §5.
 struct IfcHost {
-    int n = 0, nblk = 0, ncomp = 0;
+    int n = 0, nblk = 0, ncomp = 0, ngrp = 0;
     std::vector<int4> meta0, meta1, blk_meta;
     std::vector<double> phi;
     std::vector<int> blk_start, seg;
@@ -83,7 +83,7 @@ int analyse_ifc(const fp_ifc *f, int order, int nat, const int32_t mesh[3], IfcH
             if (at[m] < 0 || at[m] >= nat) { err = "IFC atom index out of range"; return FP_EINVAL; }
         const int32_t *RA = f->cells + (size_t)c * (order - 1) * 3 + (order - 3) * 3;   // leg A: j (3ph) / k (4ph)
         const int32_t *RB = RA + 3;                                                      // leg B: k (3ph) / l (4ph)
-        key[c] = Key(at[order - 2], at[order - 1], imod((long)RA[0] - RB[0], mesh[0]), imod((long)RA[1] - RB[1], mesh[1]),
+        key[c] = Key(at[order - 2 + FP_BLK_FORM], at[order - 1 - FP_BLK_FORM], imod((long)RA[0] - RB[0], mesh[0]), imod((long)RA[1] - RB[1], mesh[1]),
                      imod((long)RA[2] - RB[2], mesh[2]));
         blocks.emplace(key[c], 0);
     }
@@ -94,11 +94,14 @@ int analyse_ifc(const fp_ifc *f, int order, int nat, const int32_t mesh[3], IfcH
     for (auto &kv : blocks) {                                // std::map iterates sorted by (atomA, atomB, dR)
         kv.second = id;
         const Key &k = kv.first;
-        h.blk_meta[id] = make_int4(std::get<0>(k) | (std::get<1>(k) << 16), std::get<2>(k), std::get<3>(k), std::get<4>(k));
+        h.blk_meta[id] = make_int4(std::get<FP_BLK_FORM>(k) | (std::get<1 - FP_BLK_FORM>(k) << 16), std::get<2>(k), std::get<3>(k),
+                                   std::get<4>(k));           // {atomA | atomB << 16, dR}; key order = sort order
         h.seg[std::get<0>(k) * nat + std::get<1>(k) + 1]++;
         id++;
     }
     for (int i = 0; i < nat * nat; i++) h.seg[i + 1] += h.seg[i];
+    h.ngrp = 0;                                              // first-key groups with at least one block
+    for (int c = 0; c < nat; c++) h.ngrp += h.seg[(c + 1) * nat] > h.seg[c * nat];
     std::vector<int> order_idx(h.n);
     for (int c = 0; c < h.n; c++) order_idx[c] = c;
     std::stable_sort(order_idx.begin(), order_idx.end(), [&](int a, int b) { return blocks[key[a]] < blocks[key[b]]; });
@@ -161,7 +164,7 @@ int upload_ifc(fp_ctx *ctx, Bump &bump, const IfcHost &h, IfcDev &dv, cudaStream
     CU(cudaMemcpyAsync(bs, h.blk_start.data(), (h.nblk + 1) * sizeof(int), cudaMemcpyHostToDevice, st));
     CU(cudaMemcpyAsync(seg, h.seg.data(), (nat * nat + 1) * sizeof(int), cudaMemcpyHostToDevice, st));
     CU(cudaStreamSynchronize(st));                                   // host vectors go out of scope after setup
-    dv.n = h.n; dv.nblk = h.nblk; dv.ncomp = h.ncomp;
+    dv.n = h.n; dv.nblk = h.nblk; dv.ncomp = h.ncomp; dv.ngrp = h.ngrp;
     dv.cl_meta0 = m0; dv.cl_meta1 = m1; dv.phi = phi; dv.blk_start = bs; dv.blk_meta = bm; dv.seg = seg;
     return FP_OK;
 }
@@ -372,6 +375,11 @@ int fp_setup(const fp_crystal *crystal, const double *masses, const double *omeg
 int fp_destroy(fp_ctx *ctx) {
     if (!ctx) return FP_OK;
     for (auto &e : ctx->events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+    for (int i = 0; i < 2; i++) {
+        if (ctx->ev_enum[i]) cudaEventDestroy(ctx->ev_enum[i]);
+        if (ctx->ev_eval[i]) cudaEventDestroy(ctx->ev_eval[i]);
+    }
+    if (ctx->side) cudaStreamDestroy(ctx->side);
     if (ctx->pinned) cudaFreeHost(ctx->pinned);
     delete ctx;
     return FP_OK;
@@ -417,7 +425,26 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
         return fail(ctx, FP_ENOMEM, "IFC block table exceeds the shared memory of one SM");
 
     // ---- scratch budget: per-target arrays for a super-chunk of targets ------------------------------------------------
-    const size_t scratch = ctx->ws_bytes - ctx->resident;
+    const size_t scratch_all = ctx->ws_bytes - ctx->resident;
+    // ---- path: split (lists in the scratch) when half of the scratch holds two list buffers of a few hundred rows ------
+    const int64_t capw = enum_slot_entries(d);
+    const size_t row_list_bytes = (size_t)enum_warps_per_row() * ((size_t)capw * sizeof(ListEnt) + sizeof(uint32_t));
+    int64_t chunk_rows = (int64_t)std::min<size_t>((scratch_all / 2) / (2 * row_list_bytes), (size_t)1 << 20);
+    const int64_t rows_wanted = std::min<int64_t>(nt * nch * rows_per_unit, 256);
+    bool split = ctx->path == FP_PATH_SPLIT || ctx->path == FP_PATH_SPLIT_SERIAL ||
+                 (ctx->path == FP_PATH_AUTO && chunk_rows >= rows_wanted);
+    if (split && chunk_rows < 1) return fail(ctx, FP_ENOMEM, "workspace scratch too small for the process lists of one row");
+    const bool overlap = split && ctx->path != FP_PATH_SPLIT_SERIAL;
+    if (split && !ctx->side) {
+        int prio_lo = 0, prio_hi = 0;                                // enumerator CTAs take freed SM slots first: they need
+        CU(cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));    // few registers and keep the evaluator fed
+        CU(cudaStreamCreateWithPriority(&ctx->side, cudaStreamNonBlocking, prio_hi));
+        for (int i = 0; i < 2; i++) {
+            CU(cudaEventCreateWithFlags(&ctx->ev_enum[i], cudaEventDisableTiming));
+            CU(cudaEventCreateWithFlags(&ctx->ev_eval[i], cudaEventDisableTiming));
+        }
+    }
+    const size_t scratch = split ? scratch_all - 2 * (size_t)chunk_rows * row_list_bytes - 4096 : scratch_all;
     const size_t pre_per_target = (order == 3 ? (size_t)f.nblk * 9 : (size_t)f.n * 27) * sizeof(double2);
     const size_t per_target = pre_per_target + (size_t)rows_per_target * (4 + 16) + (size_t)nch * 24 + 4 + 64;
     const size_t fixed = 16 * 1024;
@@ -452,8 +479,40 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
         { ProfScope p(ctx, CAT_PRE, st);
           if (order == 3) launch_pre3(d, f, d_targets, nts, pre, st); else launch_pre4(d, f, d_targets, nts, pre, st); }
         CU(cudaGetLastError());
-        { ProfScope p(ctx, CAT_RATES, st);
-          CU(launch_rates(order, d, f, ra, nrows, pre, partial, cnt, st)); }
+        if (!split) {
+            ProfScope p(ctx, CAT_RATES, st);
+            CU(launch_rates(order, d, f, ra, nrows, pre, partial, cnt, st));
+        } else {
+            // chunks of rows through two list buffers: the enumerator of chunk k+1 (side stream) runs beside the evaluator
+            // of chunk k (caller's stream); buffer b is rewritten only after the evaluator that read it has finished
+            ListEnt *lists[2]; uint32_t *wcnt[2];
+            for (int b = 0; b < 2; b++) {
+                lists[b] = sc.take<ListEnt>((size_t)chunk_rows * enum_warps_per_row() * capw);
+                wcnt[b] = sc.take<uint32_t>((size_t)chunk_rows * enum_warps_per_row());
+                if (!lists[b] || !wcnt[b]) return fail(ctx, FP_ENOMEM, "scratch (process lists)");
+            }
+            cudaStream_t es = overlap ? ctx->side : st;
+            if (overlap) {                                           // targets and statistics are ready on st
+                CU(cudaEventRecord(ctx->ev_eval[0], st));
+                CU(cudaStreamWaitEvent(es, ctx->ev_eval[0], 0));
+            }
+            int k = 0;
+            for (int64_t r0 = 0; r0 < nrows; r0 += chunk_rows, k++) {
+                const int64_t nr = std::min(chunk_rows, nrows - r0);
+                const int b = k & 1;
+                RowArgs rc = ra; rc.row0 = r0;
+                if (overlap && k >= 2) CU(cudaStreamWaitEvent(es, ctx->ev_eval[b], 0));
+                { ProfScope p(ctx, CAT_ENUM, es);
+                  CU(launch_enum(order, d, rc, nr, capw, lists[b], wcnt[b], es)); }
+                if (overlap) {
+                    CU(cudaEventRecord(ctx->ev_enum[b], es));
+                    CU(cudaStreamWaitEvent(st, ctx->ev_enum[b], 0));
+                }
+                { ProfScope p(ctx, CAT_RATES, st);
+                  CU(launch_eval(order, d, f, rc, nr, pre, capw, lists[b], wcnt[b], partial + r0, cnt + r0, st)); }
+                if (overlap) CU(cudaEventRecord(ctx->ev_eval[b], st));
+            }
+        }
         double *g_out = loc == FP_MEM_DEVICE ? gamma + t0 * nch : o_gamma;
         double *w_out = (loc == FP_MEM_DEVICE && wp) ? wp + t0 * nch : o_wp;
         int64_t *c_out = (loc == FP_MEM_DEVICE && counts) ? counts + t0 * nch : o_cnt;
@@ -477,7 +536,8 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
             ctx->prof.processes += total;
             ctx->prof.prefiltered += (int64_t)hstat;
             ctx->prof.candidates += nrows * row_cands;
-            ctx->prof.rates_flops += (double)total * (double)f.nblk * 13.0 * 8.0;
+            ctx->prof.rates_flops += (double)total * 8.0 *
+                                     (FP_BLK_FORM ? (double)f.nblk * 12.0 + (double)f.ngrp * 3.0 : (double)f.nblk * 13.0);
         }
     }
     return FP_OK;
@@ -567,6 +627,12 @@ int fp_list4(fp_ctx *ctx, int32_t target, int32_t channel, int32_t qp, int32_t *
 }
 
 // ---- profiling ------------------------------------------------------------------------------------------------------------
+int fp_set_path(fp_ctx *ctx, int path) {
+    if (!ctx || path < FP_PATH_AUTO || path > FP_PATH_SPLIT_SERIAL) return ctx ? fail(ctx, FP_EINVAL, "unknown path") : FP_EINVAL;
+    ctx->path = path;
+    return FP_OK;
+}
+
 int fp_profile_enable(fp_ctx *ctx, int on) { if (!ctx) return FP_EINVAL; ctx->profiling = on != 0; return FP_OK; }
 
 int fp_profile_reset(fp_ctx *ctx) {
@@ -580,8 +646,8 @@ int fp_profile_reset(fp_ctx *ctx) {
 int fp_profile_get(fp_ctx *ctx, fp_profile *out) {
     if (!ctx || !out) return FP_EINVAL;
     fp_profile p = ctx->prof;
-    p.ms_precontract = p.ms_rates = p.ms_reduce = 0;
-    p.n_precontract = p.n_rates = p.n_reduce = 0;
+    p.ms_precontract = p.ms_rates = p.ms_reduce = p.ms_enum = 0;
+    p.n_precontract = p.n_rates = p.n_reduce = p.n_enum = 0;
     for (auto &e : ctx->events) {
         CU(cudaEventSynchronize(e.b));
         float ms = 0;
@@ -590,6 +656,7 @@ int fp_profile_get(fp_ctx *ctx, fp_profile *out) {
             case CAT_PRE: p.ms_precontract += ms; p.n_precontract++; break;
             case CAT_RATES: p.ms_rates += ms; p.n_rates++; break;
             case CAT_REDUCE: p.ms_reduce += ms; p.n_reduce++; break;
+            case CAT_ENUM: p.ms_enum += ms; p.n_enum++; break;
         }
     }
     *out = p;

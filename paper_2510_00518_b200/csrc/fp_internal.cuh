@@ -13,6 +13,9 @@
 
 #include "../../include/fourphonon.h"
 
+#ifndef FP_BLK_FORM
+#define FP_BLK_FORM 0         // 0: blocks sorted (atomA, atomB), V += phase*(t.Bc); 1: sorted (atomB, atomA), W_c += phase*t
+#endif
 #define FP_MAX_NB 64          // branch-mask width of the enumerator (natoms <= 21)
 #define FP_MAX_L 4096         // lcm of the mesh dimensions (1-D phase table in shared memory)
 
@@ -46,6 +49,7 @@ struct FpDev {
 // All cell offsets are stored reduced to [0,N_mu).
 struct IfcDev {
     int n, nblk, ncomp;           // clusters, blocks, 27 or 81
+    int ngrp;                     // atomB groups with at least one block (flop model of FP_BLK_FORM 1)
     const int4 *cl_meta0;         // n
     const int4 *cl_meta1;         // n (ORDER 4 only)
     const double *phi;            // n*ncomp, block-sorted
@@ -61,6 +65,9 @@ struct RowArgs {
     unsigned long long *prefiltered;   // nullable: += candidates admitted by the FP32 pre-filter (profiling)
 };
 
+// One allowed process of a row in the split path: both free legs and the row-independent part of its weight.
+struct __align__(16) ListEnt { uint32_t x, y; double w; };   // x = qA << 6 | jA,  y = qB << 6 | jB
+
 struct EventRec { int cat; cudaEvent_t a, b; };
 
 struct fp_ctx {
@@ -72,6 +79,9 @@ struct fp_ctx {
     size_t ws_bytes = 0, resident = 0;   // resident tables occupy [0, resident)
     int sm_count = 148;
     bool profiling = false;
+    int path = FP_PATH_AUTO;      // fp_set_path
+    cudaStream_t side = nullptr;  // second stream of the split path: the enumerator of chunk k+1 runs beside the
+    cudaEvent_t ev_enum[2] = {nullptr, nullptr}, ev_eval[2] = {nullptr, nullptr};   // evaluator of chunk k
     std::vector<EventRec> events;
     std::vector<cudaEvent_t> pool;
     fp_profile prof{};
@@ -80,7 +90,7 @@ struct fp_ctx {
     size_t pinned_bytes = 0;
 };
 
-enum { CAT_PRE = 0, CAT_RATES, CAT_REDUCE, CAT_N };
+enum { CAT_PRE = 0, CAT_RATES, CAT_REDUCE, CAT_ENUM, CAT_N };
 
 // ---- kernel launchers (fp_kernels.cu) --------------------------------------------------------------------------------
 void launch_tables(const FpDev &d, const double *omega, const double *eig, const double *vg, const double *masses_dev,
@@ -92,6 +102,14 @@ void launch_pre4(const FpDev &d, const IfcDev &f, const int32_t *targets, int64_
 cudaError_t launch_rates(int order, const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const double2 *pre,
                          double2 *partial, uint32_t *counts, cudaStream_t st);
 size_t rates_smem_bytes(const FpDev &d, const IfcDev &f);
+// split path (fp_rates.cu): enumerator -> process lists in the scratch -> evaluator
+int64_t enum_slot_entries(const FpDev &d);        // entries of one (row, warp) list slot
+int enum_warps_per_row();
+cudaError_t launch_enum(int order, const FpDev &d, const RowArgs &ra, int64_t nrows, int64_t capw, ListEnt *lists,
+                        uint32_t *wcnt, cudaStream_t st);
+cudaError_t launch_eval(int order, const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const double2 *pre,
+                        int64_t capw, const ListEnt *lists, const uint32_t *wcnt, double2 *partial, uint32_t *counts,
+                        cudaStream_t st);
 void launch_finalize(int order, const FpDev &d, int64_t nt, int64_t rows_per_unit, const double2 *partial,
                      const uint32_t *counts, double c_over_n, double *gamma, double *wp, int64_t *cnt, cudaStream_t st);
 void launch_kappa(const FpDev &d, const double *gamma_total, double pref, double *kappa, cudaStream_t st);

@@ -83,6 +83,18 @@ struct BlkSmem {
     int *seg;          // nat*nat+1
 };
 
+#ifndef FP_BLK_UNROLL
+#define FP_BLK_UNROLL 1
+#endif
+#ifndef FP_LATE_B
+#define FP_LATE_B 0                           // FP_BLK_FORM 1: fetch the B eigenvector when its group closes (L1 hit)
+#endif
+#ifndef FP_EVAL_PF
+#define FP_EVAL_PF 0                          // k_eval prefetches the records and eigenvectors of the next batch into L1
+#endif
+constexpr int kBlkUnroll = FP_BLK_UNROLL;
+__device__ __forceinline__ void prefetch_l1(const void *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+#if FP_BLK_FORM == 0
 // One block: u = sum_y (sum_x M[x][y] A[x]) Bc[y];  V += u * phase          (13 complex MAC = 52 DFMA)
 __device__ __forceinline__ void block_term(const double2 *M, const double2 *A, const double2 *Bc, double2 ph, double2 &V) {
     double2 u = make_double2(0.0, 0.0);
@@ -111,6 +123,7 @@ __device__ __forceinline__ double2 contract_process(const FpDev &d, const BlkSme
 #pragma unroll
             for (int c = 0; c < NAT; c++) {
                 const int b1 = bs.seg[a * NAT + c + 1];
+#pragma unroll kBlkUnroll
                 for (int b = bs.seg[a * NAT + c]; b < b1; b++) {
                     const int4 m = bs.meta[b];
                     block_term(bs.M + 9 * b, A + 3 * a, Bc + 3 * c, bs.ph[phase_idx(d, qmx, m.y, m.z, m.w)], V);
@@ -128,6 +141,7 @@ __device__ __forceinline__ double2 contract_process(const FpDev &d, const BlkSme
                 double2 Bg[3];
 #pragma unroll
                 for (int x = 0; x < 3; x++) Bg[x] = __ldg(eB + 3 * c + x);
+#pragma unroll kBlkUnroll
                 for (int b = b0; b < b1; b++) {
                     const int4 m = bs.meta[b];
                     block_term(bs.M + 9 * b, Ag, Bg, bs.ph[phase_idx(d, qmx, m.y, m.z, m.w)], V);
@@ -137,6 +151,73 @@ __device__ __forceinline__ double2 contract_process(const FpDev &d, const BlkSme
     }
     return V;
 }
+#else
+// One block: t[y] = sum_x M[x][y] A[x];  W[y] += phase * t[y]                (12 complex MAC = 48 DFMA)
+// The three t chains are independent of every other block; only the 2-deep W update is carried from block to block.
+__device__ __forceinline__ void block_term(const double2 *M, const double2 *A, double2 ph, double2 *W) {
+#pragma unroll
+    for (int y = 0; y < 3; y++) {
+        double2 t = make_double2(0.0, 0.0);
+#pragma unroll
+        for (int x = 0; x < 3; x++) cfma(t, M[3 * x + y], A[x]);
+        cfma(W[y], t, ph);
+    }
+}
+
+// V = sum_c sum_y conj(e~_B(c,y)) W_c[y],  W_c[y] = sum_{b: atomB_b = c} phi(s2 qx, dR_b) sum_x Mhat_b[x][y] A(atomA_b, x).
+// Blocks are sorted by (atomB, atomA); bs.seg[c*nat + a] is the first block of the pair.  The B eigenvector is needed only
+// when a group closes, so it is fetched there (from L1: the caller prefetched it) instead of occupying registers.
+// NAT > 0: the A eigenvector lives in registers, block loop statically split by (atomB, atomA).
+// eA points at e~_A (s2=+) or conj(e~_A) (s2=-), eB at conj(e~_B); bs.ph holds phi (s2=+) or conj(phi) (s2=-): the
+// conjugations of step 6 are table choices made once per row, not arithmetic in the loop.
+template <int NAT>
+__device__ __forceinline__ double2 contract_process(const FpDev &d, const BlkSmem &bs, const double2 *__restrict__ eA,
+                                                    const double2 *__restrict__ eB, const double2 *A, const double2 *Bc,
+                                                    int3 qmx) {
+    double2 V = make_double2(0.0, 0.0);
+    if constexpr (NAT > 0) {
+#pragma unroll
+        for (int c = 0; c < NAT; c++) {
+            double2 W[3] = {make_double2(0.0, 0.0), make_double2(0.0, 0.0), make_double2(0.0, 0.0)};
+#pragma unroll
+            for (int a = 0; a < NAT; a++) {
+                const int b1 = bs.seg[c * NAT + a + 1];
+#pragma unroll kBlkUnroll
+                for (int b = bs.seg[c * NAT + a]; b < b1; b++) {
+                    const int4 m = bs.meta[b];
+                    block_term(bs.M + 9 * b, A + 3 * a, bs.ph[phase_idx(d, qmx, m.y, m.z, m.w)], W);
+                }
+            }
+#pragma unroll
+            for (int y = 0; y < 3; y++) cfma(V, W[y], FP_LATE_B ? __ldg(eB + 3 * c + y) : Bc[3 * c + y]);
+        }
+    } else {
+        const int nat = d.nat;
+        for (int c = 0; c < nat; c++) {
+            if (bs.seg[c * nat] == bs.seg[(c + 1) * nat]) continue;
+            double2 Bg[3];                                           // issued here, consumed after the group's blocks
+#pragma unroll
+            for (int y = 0; y < 3; y++) Bg[y] = __ldg(eB + 3 * c + y);
+            double2 W[3] = {make_double2(0.0, 0.0), make_double2(0.0, 0.0), make_double2(0.0, 0.0)};
+            for (int a = 0; a < nat; a++) {
+                const int b0 = bs.seg[c * nat + a], b1 = bs.seg[c * nat + a + 1];
+                if (b0 == b1) continue;
+                double2 Ag[3];
+#pragma unroll
+                for (int x = 0; x < 3; x++) Ag[x] = __ldg(eA + 3 * a + x);
+#pragma unroll kBlkUnroll
+                for (int b = b0; b < b1; b++) {
+                    const int4 m = bs.meta[b];
+                    block_term(bs.M + 9 * b, Ag, bs.ph[phase_idx(d, qmx, m.y, m.z, m.w)], W);
+                }
+            }
+#pragma unroll
+            for (int y = 0; y < 3; y++) cfma(V, W[y], Bg[y]);
+        }
+    }
+    return V;
+}
+#endif
 
 
 // ---------------------------------------------------------------------------------------------------------------------
@@ -144,9 +225,6 @@ __device__ __forceinline__ double2 contract_process(const FpDev &d, const BlkSme
 // ---------------------------------------------------------------------------------------------------------------------
 #ifndef FP_MINB
 #define FP_MINB 4                             // resident CTAs per SM the register allocation targets
-#endif
-#ifndef FP_PREFETCH
-#define FP_PREFETCH 0                         // stage 2 prefetches the records and eigenvectors of its survivors into L1
 #endif
 constexpr int RT = 128;                       // threads per row CTA
 constexpr int RW = RT / 32;                   // warps
@@ -177,7 +255,15 @@ __device__ __forceinline__ void eval_process(const FpDev &d, const BlkSmem &bs, 
     double2 A[3 * (NAT > 0 ? NAT : 1)], Bc[3 * (NAT > 0 ? NAT : 1)];
     if constexpr (NAT > 0) {
 #pragma unroll
-        for (int c = 0; c < 3 * NAT; c++) { A[c] = __ldg(eA + c); Bc[c] = __ldg(eB + c); }
+        for (int c = 0; c < 3 * NAT; c++) A[c] = __ldg(eA + c);
+#if FP_BLK_FORM == 1 && FP_LATE_B
+#if !FP_EVAL_PF
+        prefetch_l1(eB); prefetch_l1(eB + 3 * NAT - 1);
+#endif
+#else
+#pragma unroll
+        for (int c = 0; c < 3 * NAT; c++) Bc[c] = __ldg(eB + c);
+#endif
     }
     // the decision, in the pinned arithmetic
     const double sig = sigma_pinned(d, a, b);
@@ -202,10 +288,6 @@ __device__ __forceinline__ void eval_process(const FpDev &d, const BlkSmem &bs, 
     }
 }
 
-#if FP_PREFETCH
-__device__ __forceinline__ void prefetch_l1(const void *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
-#endif
-
 // FP32 pre-filter, stage 2, of one candidate code (table recf): Delta_f^2 <= K1 |u_a - u_b|_f^2 + C2
 __device__ __forceinline__ bool prefilter2(const FpDev &d, const Row &row, float basef, uint32_t code, uint2 &ent) {
     const int qx = (int)(code >> 12), ja = (int)((code >> 6) & 63u), jb = (int)(code & 63u);
@@ -215,18 +297,7 @@ __device__ __forceinline__ bool prefilter2(const FpDev &d, const Row &row, float
     const float dl = (row.s2 > 0 ? basef + A.x : basef - A.x) - B.x;
     const float dx = A.y - B.y, dy = A.z - B.z, dz = A.w - B.w;
     const float s = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-    const bool pass = dl * dl <= fmaf(d.pfK1, s, d.pfC2);
-#if FP_PREFETCH
-    if (pass) {
-        const size_t pa = (size_t)qx * d.nb + ja, pb = (size_t)ql * d.nb + jb;
-        const char *ea = reinterpret_cast<const char *>((row.s2 > 0 ? d.evec : d.evecc) + pa * d.nb);
-        const char *eb = reinterpret_cast<const char *>(d.evecc + pb * d.nb);
-        const int last = d.nb * 16 - 16;
-        prefetch_l1(d.rec + pa); prefetch_l1(d.rec + pb);
-        prefetch_l1(ea); prefetch_l1(ea + last); prefetch_l1(eb); prefetch_l1(eb + last);
-    }
-#endif
-    return pass;
+    return dl * dl <= fmaf(d.pfK1, s, d.pfC2);
 }
 
 // No candidate of the row can pass the window: |Delta| <= ncut sigma <= n_a + n_b <= 2 nmax for every allowed process,
@@ -238,29 +309,17 @@ __device__ __forceinline__ bool row_is_empty(const FpDev &d, const Row &row) {
     return dmin > w2 || dmax < -w2;
 }
 
-template <int ORDER, int NAT, int TILE>
-__global__ void __launch_bounds__(RT, FP_MINB) k_rates(FpDev d, IfcDev f, RowArgs ra, const double2 *pre, double2 *partial,
-                                                 uint32_t *counts) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ double red[32];
-    __shared__ unsigned redc[32];
-    __shared__ int tailn[RW];
-    const int64_t r = blockIdx.x;
-    const Row row = make_row<ORDER>(d, ra, ra.row0 + r);
-    if (!row.valid || row_is_empty(d, row)) {                         // item 8: zero modes are never a leg
-        if (threadIdx.x == 0) { partial[r] = make_double2(0.0, 0.0); counts[r] = 0; }
-        return;
-    }
-    BlkSmem bs;                                                       // layout mirrored by rates_smem_bytes()
+// Shared-memory tables of one row (layout mirrored by tables_smem_bytes()): Mhat, phases, level-1 eigenvector, block
+// metadata, (atomA, atomB) segments.  Returns the first free byte after them.
+template <int ORDER>
+__device__ __forceinline__ unsigned char *setup_row_tables(const FpDev &d, const IfcDev &f, const Row &row,
+                                                           const double2 *pre, unsigned char *smem_raw, BlkSmem &bs,
+                                                           RowWeights &rw) {
     bs.M = reinterpret_cast<double2 *>(smem_raw);
     bs.ph = bs.M + 9 * f.nblk;
     double2 *e1 = bs.ph + d.L;                                        // nb entries (level 1 of ORDER 4)
     bs.meta = reinterpret_cast<int4 *>(e1 + d.nb);
     bs.seg = reinterpret_cast<int *>(bs.meta + f.nblk);
-    uint2 *evq = reinterpret_cast<uint2 *>(bs.seg + ((d.nat * d.nat + 1 + 3) & ~3));   // RW*QCAP, then RW*32 (tails)
-    uint2 *tailbuf = evq + RW * QCAP;
-    uint32_t *pendq = reinterpret_cast<uint32_t *>(tailbuf + RW * 32);                // RW*PCAP
-
     for (int i = threadIdx.x; i < f.nblk; i += RT) bs.meta[i] = f.blk_meta[i];
     for (int i = threadIdx.x; i <= d.nat * d.nat; i += RT) bs.seg[i] = f.seg[i];
     if (ORDER == 3) {
@@ -299,8 +358,6 @@ __global__ void __launch_bounds__(RT, FP_MINB) k_rates(FpDev d, IfcDev f, RowArg
         bs.ph[i] = p;
     }
     __syncthreads();
-
-    RowWeights rw;
     rw.wrow = d.rec[row.lam].omega;
     rw.occ_row = 1.0;
     if (ORDER == 4) {
@@ -308,6 +365,91 @@ __global__ void __launch_bounds__(RT, FP_MINB) k_rates(FpDev d, IfcDev f, RowArg
         rw.wrow *= d.rec[row.lam1].omega;
         rw.occ_row = (row.s1 > 0 ? 1.0 + f1 : f1) / d.occ[row.lam];
     }
+    return reinterpret_cast<unsigned char *>(bs.seg + ((d.nat * d.nat + 1 + 3) & ~3));
+}
+
+// FP32 pre-filter, stage 1, of one sub-tile (32 q-points x TILE x TILE branch pairs, table recn): each lane owns one
+// q-point and admits a pair iff |Delta_f| <= n'_a + n'_b (sigma <= cs(|u_a| + |u_b|)); survivors are appended, in
+// candidate order, to the warp's pending queue.  Returns the new queue length (warp-uniform).
+template <int TILE>
+__device__ __forceinline__ int stage1_step(const FpDev &d, const Row &row, float basef, int tile, int ja0, int jb0,
+                                           int lane, uint32_t *pend, int wp) {
+    const float fnan = __int_as_float(0x7fc00000);
+    const int qx = (tile << 5) + lane;
+    const bool inq = qx < d.N;
+    const int qs = inq ? qx : 0;
+    const int ql = q_index(d, q_add(d, row.qb, row.s2, unpack_qc(d.qc[qs])));
+    const float2 *pa = d.recn + (size_t)qs * d.nb + ja0, *pb = d.recn + (size_t)ql * d.nb + jb0;
+    float lo[TILE], hi[TILE];
+#pragma unroll
+    for (int i = 0; i < TILE; i++) {
+        const float2 A = __ldg(pa + i);                               // omega_f = NaN for zero modes: never admitted
+        const float ba = inq ? (row.s2 > 0 ? basef + A.x : basef - A.x) : fnan;
+        lo[i] = ba - A.y; hi[i] = ba + A.y;
+    }
+    uint64_t mask = 0;
+#pragma unroll
+    for (int k = 0; k < TILE; k++) {
+        const float2 B = __ldg(pb + k);
+        const float bl = B.x - B.y, bh = B.x + B.y;
+#pragma unroll
+        for (int i = 0; i < TILE; i++)
+            if (bl <= hi[i] && bh >= lo[i]) mask |= 1ull << (8 * i + k);
+    }
+    const unsigned c = __popcll(mask);                                // ordered append to the pending queue
+    unsigned incl = c;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        unsigned v = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += v;
+    }
+    unsigned pos = wp + incl - c;
+    while (mask) {
+        const int bit = __ffsll((long long)mask) - 1;
+        mask &= mask - 1;
+        pend[pos++] = pack_code(qx, ja0 + (bit >> 3), jb0 + (bit & 7));
+    }
+    return wp + (int)__shfl_sync(0xffffffffu, incl, 31);
+}
+
+// sub-tile decomposition of the enumeration: step -> (q-tile, ja0, jb0)
+template <int TILE, bool ONE_SUB>
+struct Steps {
+    int nsub, nsteps;
+    __device__ __forceinline__ Steps(const FpDev &d) {
+        nsub = ONE_SUB ? 1 : d.nb / TILE;
+        nsteps = ((d.N + 31) >> 5) * nsub * nsub;
+    }
+    __device__ __forceinline__ void decode(int step, int &tile, int &ja0, int &jb0) const {
+        if (ONE_SUB) { tile = step; ja0 = 0; jb0 = 0; return; }
+        tile = step / (nsub * nsub);
+        const int sub = step - tile * nsub * nsub;
+        ja0 = (sub / nsub) * TILE; jb0 = (sub - (sub / nsub) * nsub) * TILE;
+    }
+};
+
+// ---------------------------------------------------------------------------------------------------------------------
+// fused path: enumerate -> shared-memory queues -> evaluate, one CTA per row (used when the scratch is too small for
+// process lists; the process lists of Algorithm 3, live and die in shared memory)
+// ---------------------------------------------------------------------------------------------------------------------
+template <int ORDER, int NAT, int TILE>
+__global__ void __launch_bounds__(RT, FP_MINB) k_rates(FpDev d, IfcDev f, RowArgs ra, const double2 *pre, double2 *partial,
+                                                 uint32_t *counts) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ double red[32];
+    __shared__ unsigned redc[32];
+    __shared__ int tailn[RW];
+    const int64_t r = blockIdx.x;
+    const Row row = make_row<ORDER>(d, ra, ra.row0 + r);
+    if (!row.valid || row_is_empty(d, row)) {                         // item 8: zero modes are never a leg
+        if (threadIdx.x == 0) { partial[r] = make_double2(0.0, 0.0); counts[r] = 0; }
+        return;
+    }
+    BlkSmem bs;
+    RowWeights rw;
+    uint2 *evq = reinterpret_cast<uint2 *>(setup_row_tables<ORDER>(d, f, row, pre, smem_raw, bs, rw));   // RW*QCAP
+    uint2 *tailbuf = evq + RW * QCAP;                                                  // RW*32 (merged tails)
+    uint32_t *pendq = reinterpret_cast<uint32_t *>(tailbuf + RW * 32);                // RW*PCAP
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     uint32_t *pend = pendq + warp * PCAP;                             // stage-1 survivors of this warp
@@ -317,16 +459,11 @@ __global__ void __launch_bounds__(RT, FP_MINB) k_rates(FpDev d, IfcDev f, RowArg
     unsigned cnt = 0, nadm = 0;
 
     // ---- one loop, one evaluation site: evaluate a full batch if one is queued, else refill the queue -------------------
-    //   enumerate a sub-tile (32 q-points x TILE x TILE branch pairs) with the FP32 pre-filter, two stages:
-    //     stage 1 (2 compares per pair, table recn):          |Delta_f| <= n'_a + n'_b   (sigma <= cs(|u_a| + |u_b|))
-    //     stage 2 (warp-cooperative on the survivors, recf):  Delta_f^2 <= K1 |u_a - u_b|_f^2 + C2
-    //   Both admit every candidate the pinned FP64 decision allows, which alone decides.
+    //   stage 1 (stage1_step) and stage 2 (prefilter2) admit every candidate the pinned FP64 decision allows
+    //   (DESIGN.md §5.2), which alone decides.
     const float basef = (float)row.Obase;
-    const float fnan = __int_as_float(0x7fc00000);
-    const int ntile = (d.N + 31) >> 5;
     constexpr bool ONE_SUB = (NAT > 0 && 3 * NAT == TILE);            // nb == TILE: one sub-tile per q-tile
-    const int nsub = ONE_SUB ? 1 : d.nb / TILE;
-    const int nsteps = ntile * nsub * nsub;
+    const Steps<TILE, ONE_SUB> steps(d);
     int step = warp, phase = 0, tbase = 0, total = 0;                 // phase 0 enumerate, 1 flush pend, 2 merged tails
     for (;;) {
         __syncwarp();
@@ -357,46 +494,11 @@ __global__ void __launch_bounds__(RT, FP_MINB) k_rates(FpDev d, IfcDev f, RowArg
             continue;
         }
         if (phase == 0) {
-            if (step >= nsteps) { phase = 1; continue; }
-            const int tile = ONE_SUB ? step : step / (nsub * nsub), sub = ONE_SUB ? 0 : step - tile * nsub * nsub;
-            const int ja0 = ONE_SUB ? 0 : (sub / nsub) * TILE, jb0 = ONE_SUB ? 0 : (sub - (sub / nsub) * nsub) * TILE;
+            if (step >= steps.nsteps) { phase = 1; continue; }
+            int tile, ja0, jb0;
+            steps.decode(step, tile, ja0, jb0);
             step += RW;
-            const int qx = (tile << 5) + lane;
-            const bool inq = qx < d.N;
-            const int qs = inq ? qx : 0;
-            const int ql = q_index(d, q_add(d, row.qb, row.s2, unpack_qc(d.qc[qs])));
-            const float2 *pa = d.recn + (size_t)qs * d.nb + ja0, *pb = d.recn + (size_t)ql * d.nb + jb0;
-            float lo[TILE], hi[TILE];
-#pragma unroll
-            for (int i = 0; i < TILE; i++) {
-                const float2 A = __ldg(pa + i);                       // omega_f = NaN for zero modes: never admitted
-                const float ba = inq ? (row.s2 > 0 ? basef + A.x : basef - A.x) : fnan;
-                lo[i] = ba - A.y; hi[i] = ba + A.y;
-            }
-            uint64_t mask = 0;
-#pragma unroll
-            for (int k = 0; k < TILE; k++) {
-                const float2 B = __ldg(pb + k);
-                const float bl = B.x - B.y, bh = B.x + B.y;
-#pragma unroll
-                for (int i = 0; i < TILE; i++)
-                    if (bl <= hi[i] && bh >= lo[i]) mask |= 1ull << (8 * i + k);
-            }
-            // ordered append to the pending queue
-            const unsigned c = __popcll(mask);
-            unsigned incl = c;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                unsigned v = __shfl_up_sync(0xffffffffu, incl, o);
-                if (lane >= o) incl += v;
-            }
-            unsigned pos = wp + incl - c;
-            while (mask) {
-                const int bit = __ffsll((long long)mask) - 1;
-                mask &= mask - 1;
-                pend[pos++] = pack_code(qx, ja0 + (bit >> 3), jb0 + (bit & 7));
-            }
-            wp += __shfl_sync(0xffffffffu, incl, 31);
+            wp = stage1_step<TILE>(d, row, basef, tile, ja0, jb0, lane, pend, wp);
             continue;
         }
         // phase 1 with pend empty and fewer than 32 queued: merge the leftovers of all warps so that at most one batch
@@ -425,6 +527,139 @@ __global__ void __launch_bounds__(RT, FP_MINB) k_rates(FpDev d, IfcDev f, RowArg
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------------
+// split path (the default): process lists in HBM, Algorithm 3 -> Algorithm 4 of the paper with both
+// halves on the device.  The enumerator needs ~40 registers and no FP64 pipe, the evaluator 128 registers and little
+// else: as separate kernels each runs at its own occupancy, and (on two streams) the enumerator of the next chunk of
+// rows fills the issue slots the FP64-bound evaluator leaves empty.
+//
+// List layout: every (row, warp) owns a slot of capw entries (capw = all candidates the warp can meet, so nothing can
+// overflow; untouched slot space costs no traffic); wcnt[row*RW + warp] is the number of entries written.  Entry order
+// inside a slot is the enumerator's (deterministic), so sums are reproducible run to run.
+// ---------------------------------------------------------------------------------------------------------------------
+static_assert(RW == 4, "k_eval reads the four warp counts of a row as one uint4");
+
+// Enumerator: stage 1 and 2 of the FP32 pre-filter, then -- for the survivors only -- the pinned FP64 decision
+// (SURVEY.md §8(c) step 3), which alone determines what is written, and the row-independent part of the
+// weight (a7).  With ~48 registers per thread ten CTAs fit on an SM, which hides the gather latency of the decision.
+template <int ORDER, int TILE, bool ONE_SUB>
+__global__ void __launch_bounds__(RT, 8) k_enum(FpDev d, RowArgs ra, int64_t capw, ListEnt *lists, uint32_t *wcnt) {
+    __shared__ uint32_t pendq[RW * PCAP];
+    const int64_t r = blockIdx.x;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const Row row = make_row<ORDER>(d, ra, ra.row0 + r);
+    unsigned nout = 0, nadm = 0;
+    if (row.valid && !row_is_empty(d, row)) {                         // item 8: zero modes are never a leg
+        ListEnt *out = lists + ((size_t)r * RW + warp) * (size_t)capw;
+        uint32_t *pend = pendq + warp * PCAP;
+        const float basef = (float)row.Obase;
+        const Steps<TILE, ONE_SUB> steps(d);
+        int wp = 0;
+        for (int step = warp; step < steps.nsteps; step += RW) {
+            int tile, ja0, jb0;
+            steps.decode(step, tile, ja0, jb0);
+            wp = stage1_step<TILE>(d, row, basef, tile, ja0, jb0, lane, pend, wp);
+            __syncwarp();
+            const bool last = step + RW >= steps.nsteps;
+            while (wp >= 32 || (last && wp > 0)) {                    // stage 2, 32 pending candidates at a time
+                const int n = wp < 32 ? wp : 32;
+                wp -= n;
+                const bool in = lane < n;
+                const uint32_t c2 = pend[wp + (in ? lane : 0)];
+                uint2 e2;
+                const bool pass = prefilter2(d, row, basef, c2, e2) && in;
+                bool ok = false;
+                double w = 0.0;
+                if (pass) {                                           // stage 3: the decision, in the pinned arithmetic
+                    const int p = (int)(e2.x >> 6) * d.nb + (int)(e2.x & 63u), lamB = (int)(e2.y >> 6) * d.nb + (int)(e2.y & 63u);
+                    const ModeRec a = load_rec(d.rec + p), b = load_rec(d.rec + lamB);
+                    const double fa = __ldg(d.occ + p), fb = __ldg(d.occ + lamB);
+                    const double sig = sigma_pinned(d, a, b);
+                    const double delta = __dsub_rn(row.s2 > 0 ? __dadd_rn(row.Obase, a.omega) : __dsub_rn(row.Obase, a.omega), b.omega);
+                    ok = a.omega != 0.0 && b.omega != 0.0 && sig > 0.0 && fabs(delta) <= __dmul_rn(d.ncut, sig);
+                    // weight without the row factors: occ(f_A, f_B) g / (omega_A omega_B),  g = exp(-(Delta/sigma)^2)/(sigma sqrt(pi))
+                    const double W = a.omega * b.omega;
+                    const double t = 1.0 / (sig * W);
+                    const double rr = delta * (t * W);
+                    double occ;
+                    if (ORDER == 3) occ = row.s2 > 0 ? (fa - fb) : (fa + fb + 1.0);
+                    else occ = (row.s2 > 0 ? 1.0 + fa : fa) * fb;
+                    w = occ * (exp(-(rr * rr)) * t * 0.56418958354775628695);   // 1/sqrt(pi)
+                }
+                const unsigned bal = __ballot_sync(0xffffffffu, ok);
+                if (ok) {
+                    ListEnt e; e.x = e2.x; e.y = e2.y; e.w = w;
+                    out[nout + __popc(bal & ((1u << lane) - 1u))] = e;
+                }
+                nout += __popc(bal);
+                nadm += pass ? 1u : 0u;
+            }
+            __syncwarp();
+        }
+    }
+    if (lane == 0) wcnt[r * RW + warp] = nout;
+    if (ra.prefiltered) {                                             // profiling only: pre-filter survivors
+        for (int o = 16; o > 0; o >>= 1) nadm += __shfl_down_sync(0xffffffffu, nadm, o);
+        if (lane == 0 && nadm) atomicAdd(ra.prefiltered, (unsigned long long)nadm);
+    }
+}
+
+// Evaluator: |V|^2 of every listed process (level-2 contraction) and the row sums.  Every entry is an allowed process,
+// so the row count is the list length; the row factors of the weight (1/omega[omega'], occupation of lambda') multiply
+// the sums once.
+template <int ORDER, int NAT>
+__global__ void __launch_bounds__(RT, FP_MINB) k_eval(FpDev d, IfcDev f, RowArgs ra, const double2 *pre, int64_t capw,
+                                                      const ListEnt *lists, const uint32_t *wcnt, double2 *partial,
+                                                      uint32_t *counts) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ double red[32];
+    const int64_t r = blockIdx.x;
+    const uint4 wc = __ldg(reinterpret_cast<const uint4 *>(wcnt) + r);
+    const unsigned p1 = wc.x, p2 = p1 + wc.y, p3 = p2 + wc.z, total = p3 + wc.w;
+    if (total == 0) {
+        if (threadIdx.x == 0) { partial[r] = make_double2(0.0, 0.0); counts[r] = 0; }
+        return;
+    }
+    const Row row = make_row<ORDER>(d, ra, ra.row0 + r);
+    BlkSmem bs;
+    RowWeights rw;
+    setup_row_tables<ORDER>(d, f, row, pre, smem_raw, bs, rw);
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const ListEnt *slot = lists + (size_t)r * RW * (size_t)capw;
+    // the four slots of the row read as one list: entry i lives in slot w = #{k : i >= p_k} at offset i - p_w
+    auto fetch = [&](unsigned i) -> ListEnt {
+        const unsigned w = (i >= p1) + (i >= p2) + (i >= p3);
+        const unsigned off = i - (w == 0 ? 0u : w == 1 ? p1 : w == 2 ? p2 : p3);
+        const uint4 v = __ldg(reinterpret_cast<const uint4 *>(slot + (size_t)w * (size_t)capw + off));
+        ListEnt e; e.x = v.x; e.y = v.y; e.w = __hiloint2double((int)v.w, (int)v.z);
+        return e;
+    };
+    double sG = 0.0, sW = 0.0;
+    for (unsigned base = warp * 32; base < total; base += RT) {       // batch b of the row goes to warp b mod RW
+        const bool act = base + lane < total;
+        const ListEnt e = fetch(act ? base + lane : base);
+        const int qx = (int)(e.x >> 6);
+        const int p = qx * d.nb + (int)(e.x & 63u), lamB = (int)(e.y >> 6) * d.nb + (int)(e.y & 63u);
+        const double2 *eA = (row.s2 > 0 ? d.evec : d.evecc) + (size_t)p * d.nb, *eB = d.evecc + (size_t)lamB * d.nb;
+        const int3 xc = unpack_qc(__ldg(d.qc + qx));
+        double2 A[3 * (NAT > 0 ? NAT : 1)], Bc[3 * (NAT > 0 ? NAT : 1)];
+        if constexpr (NAT > 0) {
+#pragma unroll
+            for (int c = 0; c < 3 * NAT; c++) { A[c] = __ldg(eA + c); Bc[c] = __ldg(eB + c); }
+        }
+        const double2 V = contract_process<NAT>(d, bs, eA, eB, A, Bc, premul(d, xc));
+        if (act) {
+            sW += e.w;
+            sG = fma(e.w, V.x * V.x + V.y * V.y, sG);
+        }
+    }
+    const double rowfac = rw.occ_row / rw.wrow;
+    const double tG = block_sum<double>(sG, red);
+    const double tW = block_sum<double>(sW, red);
+    if (threadIdx.x == 0) { partial[r] = make_double2(rowfac * tG, rowfac * tW); counts[r] = total; }
+}
+
 }  // namespace
 
 // ---------------------------------------------------------------------------------------------------------------------
@@ -437,23 +672,32 @@ void launch_pre4(const FpDev &d, const IfcDev &f, const int32_t *targets, int64_
     if (nt > 0) k_pre4<<<(unsigned)nt, 256, 0, st>>>(d, f, targets, t0);
 }
 
+static size_t tables_smem_bytes(const FpDev &d, const IfcDev &f) {
+    return (size_t)f.nblk * 9 * sizeof(double2) + (size_t)d.L * sizeof(double2) + (size_t)d.nb * sizeof(double2) +
+           (size_t)f.nblk * sizeof(int4) + (size_t)((d.nat * d.nat + 1 + 3) & ~3) * sizeof(int);
+}
 size_t rates_smem_bytes(const FpDev &d, const IfcDev &f) {
-    size_t b = (size_t)f.nblk * 9 * sizeof(double2) + (size_t)d.L * sizeof(double2) + (size_t)d.nb * sizeof(double2) +
-               (size_t)f.nblk * sizeof(int4) + (size_t)((d.nat * d.nat + 1 + 3) & ~3) * sizeof(int) +
-               (size_t)(RW * QCAP + RW * 32) * sizeof(uint2) + (size_t)(RW * PCAP) * sizeof(uint32_t);
+    size_t b = tables_smem_bytes(d, f) + (size_t)(RW * QCAP + RW * 32) * sizeof(uint2) + (size_t)(RW * PCAP) * sizeof(uint32_t);
     return (b + 15) & ~(size_t)15;
+}
+
+template <typename K>
+static cudaError_t opt_in_smem(K kernel, size_t smem, size_t &granted) {   // opt-in limit is 227 KB minus the static part
+    if (smem > 48 * 1024 && smem > granted) {
+        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        granted = smem;
+    }
+    return cudaSuccess;
 }
 
 template <int ORDER, int NAT, int TILE>
 static cudaError_t launch_rates_t(const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const double2 *pre,
                                   double2 *partial, uint32_t *counts, cudaStream_t st) {
     const size_t smem = rates_smem_bytes(d, f);
-    static size_t attr_smem = 0;                                     // opt-in limit is 227 KB minus the static part
-    if (smem > 48 * 1024 && smem > attr_smem) {
-        cudaError_t e = cudaFuncSetAttribute(k_rates<ORDER, NAT, TILE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        attr_smem = smem;
-    }
+    static size_t granted = 0;
+    cudaError_t e = opt_in_smem(k_rates<ORDER, NAT, TILE>, smem, granted);
+    if (e != cudaSuccess) return e;
     k_rates<ORDER, NAT, TILE><<<(unsigned)nrows, RT, smem, st>>>(d, f, ra, pre, partial, counts);
     return cudaGetLastError();
 }
@@ -471,5 +715,58 @@ cudaError_t launch_rates(int order, const FpDev &d, const IfcDev &f, const RowAr
     if (d.nat == 1) return launch_rates_t<4, 1, 3>(FP_ARGS);
     if (d.nat == 2) return launch_rates_t<4, 2, 6>(FP_ARGS);
     return t6 ? launch_rates_t<4, 0, 6>(FP_ARGS) : launch_rates_t<4, 0, 3>(FP_ARGS);
+#undef FP_ARGS
+}
+
+// ---- split path ------------------------------------------------------------------------------------------------------
+// entries one warp of k_enum can write for one row: its share of the sub-tile steps, every candidate admitted
+int64_t enum_slot_entries(const FpDev &d) {
+    const int tile = d.nb % 6 == 0 ? 6 : 3;
+    const int64_t nsub = d.nb / tile, nsteps = (int64_t)((d.N + 31) >> 5) * nsub * nsub;
+    return (nsteps + RW - 1) / RW * 32 * tile * tile;
+}
+int enum_warps_per_row() { return RW; }
+
+cudaError_t launch_enum(int order, const FpDev &d, const RowArgs &ra, int64_t nrows, int64_t capw, ListEnt *lists,
+                        uint32_t *wcnt, cudaStream_t st) {
+    if (nrows <= 0) return cudaSuccess;
+    const unsigned g = (unsigned)nrows;
+#define FP_ENUM(O, T, S) k_enum<O, T, S><<<g, RT, 0, st>>>(d, ra, capw, lists, wcnt)
+    if (order == 3) {
+        if (d.nb == 6) FP_ENUM(3, 6, true); else if (d.nb == 3) FP_ENUM(3, 3, true);
+        else if (d.nb % 6 == 0) FP_ENUM(3, 6, false); else FP_ENUM(3, 3, false);
+    } else {
+        if (d.nb == 6) FP_ENUM(4, 6, true); else if (d.nb == 3) FP_ENUM(4, 3, true);
+        else if (d.nb % 6 == 0) FP_ENUM(4, 6, false); else FP_ENUM(4, 3, false);
+    }
+#undef FP_ENUM
+    return cudaGetLastError();
+}
+
+template <int ORDER, int NAT>
+static cudaError_t launch_eval_t(const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const double2 *pre,
+                                 int64_t capw, const ListEnt *lists, const uint32_t *wcnt, double2 *partial,
+                                 uint32_t *counts, cudaStream_t st) {
+    const size_t smem = (tables_smem_bytes(d, f) + 15) & ~(size_t)15;
+    static size_t granted = 0;
+    cudaError_t e = opt_in_smem(k_eval<ORDER, NAT>, smem, granted);
+    if (e != cudaSuccess) return e;
+    k_eval<ORDER, NAT><<<(unsigned)nrows, RT, smem, st>>>(d, f, ra, pre, capw, lists, wcnt, partial, counts);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_eval(int order, const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const double2 *pre,
+                        int64_t capw, const ListEnt *lists, const uint32_t *wcnt, double2 *partial, uint32_t *counts,
+                        cudaStream_t st) {
+    if (nrows <= 0) return cudaSuccess;
+#define FP_ARGS d, f, ra, nrows, pre, capw, lists, wcnt, partial, counts, st
+    if (order == 3) {
+        if (d.nat == 1) return launch_eval_t<3, 1>(FP_ARGS);
+        if (d.nat == 2) return launch_eval_t<3, 2>(FP_ARGS);
+        return launch_eval_t<3, 0>(FP_ARGS);
+    }
+    if (d.nat == 1) return launch_eval_t<4, 1>(FP_ARGS);
+    if (d.nat == 2) return launch_eval_t<4, 2>(FP_ARGS);
+    return launch_eval_t<4, 0>(FP_ARGS);
 #undef FP_ARGS
 }

@@ -23,6 +23,11 @@ def fp():
     return fp
 
 
+def PATHS(fp):
+    """fused (lists in shared memory) and split (enumerator -> lists in the scratch -> evaluator, two streams)"""
+    return (fp.FP_PATH_FUSED, fp.FP_PATH_SPLIT)
+
+
 def _oracle(inp, **kw):
     from oracle.oracle import Oracle
     return Oracle(inp, **kw)
@@ -48,22 +53,28 @@ def assert_rates_close(got, ref, what):
 def check3(fp, inp, targets, **kw):
     orc = _oracle(inp, **{k: v for k, v in kw.items() if k in ("ncut", "sigma_const", "T", "scale")})
     og, ow, oc = orc.rates3(targets)
-    with fp.Context.from_inputs(inp, scratch_bytes=kw.pop("scratch_bytes", 64 << 20), **kw) as ctx:
-        g, w, c = ctx.rates3(targets)
-    assert np.array_equal(c, oc), "3ph process counts are not bit-exact"
-    assert_rates_close(g, og, "Gamma3")
-    assert_rates_close(w, ow, "WP3")
+    scratch = kw.pop("scratch_bytes", 64 << 20)
+    for path in PATHS(fp):                                            # both execution paths meet the same bar
+        with fp.Context.from_inputs(inp, scratch_bytes=scratch, **kw) as ctx:
+            ctx.set_path(path)
+            g, w, c = ctx.rates3(targets)
+        assert np.array_equal(c, oc), f"3ph process counts are not bit-exact (path {path})"
+        assert_rates_close(g, og, f"Gamma3 (path {path})")
+        assert_rates_close(w, ow, f"WP3 (path {path})")
     return g, c
 
 
 def check4(fp, inp, targets, qp=(0, None), **kw):
     orc = _oracle(inp, **{k: v for k, v in kw.items() if k in ("ncut", "sigma_const", "T", "scale")})
     og, ow, oc = orc.rates4(targets, qp[0], qp[1])
-    with fp.Context.from_inputs(inp, scratch_bytes=kw.pop("scratch_bytes", 64 << 20), **kw) as ctx:
-        g, w, c = ctx.rates4(targets, qp[0], qp[1])
-    assert np.array_equal(c, oc), "4ph process counts are not bit-exact"
-    assert_rates_close(g, og, "Gamma4")
-    assert_rates_close(w, ow, "WP4")
+    scratch = kw.pop("scratch_bytes", 64 << 20)
+    for path in PATHS(fp):
+        with fp.Context.from_inputs(inp, scratch_bytes=scratch, **kw) as ctx:
+            ctx.set_path(path)
+            g, w, c = ctx.rates4(targets, qp[0], qp[1])
+        assert np.array_equal(c, oc), f"4ph process counts are not bit-exact (path {path})"
+        assert_rates_close(g, og, f"Gamma4 (path {path})")
+        assert_rates_close(w, ow, f"WP4 (path {path})")
     return g, c
 
 
@@ -191,18 +202,40 @@ def test_small_scratch_splits_targets_and_gives_identical_results(fp):
     """A scratch that holds a few targets at a time forces the bounded-memory loop (Algorithm 5)."""
     inp = fp_inputs.make_tiny("diamond", mesh=(3, 3, 3))
     t = inp.targets4[6:30]
-    with fp.Context.from_inputs(inp, scratch_bytes=64 << 20) as big:
-        big.profile_enable(True)
-        g, w, c = big.rates4(t)
-        assert big.profile_get().n_rates == 1
-    with fp.Context.from_inputs(inp, scratch_bytes=512 << 10) as small:
-        small.profile_enable(True)
-        gs, ws, cs = small.rates4(t)
-        p = small.profile_get()
-        assert p.n_rates > 1
-        assert p.processes == int(cs.sum()) and p.prefiltered >= p.processes
-        assert p.candidates == len(t) * 3 * inp.nq ** 2 * inp.nb ** 3
-    assert np.array_equal(c, cs) and np.array_equal(g, gs) and np.array_equal(w, ws)
+    for path in PATHS(fp):                                            # chunking never changes a row's arithmetic
+        with fp.Context.from_inputs(inp, scratch_bytes=256 << 20) as big:
+            big.set_path(path)
+            big.profile_enable(True)
+            g, w, c = big.rates4(t)
+            n_big = big.profile_get().n_rates
+            assert n_big == 1 or path != fp.FP_PATH_FUSED
+        with fp.Context.from_inputs(inp, scratch_bytes=512 << 10) as small:
+            small.set_path(path)
+            small.profile_enable(True)
+            gs, ws, cs = small.rates4(t)
+            p = small.profile_get()
+            assert p.n_rates > n_big
+            assert p.processes == int(cs.sum()) and p.prefiltered >= p.processes
+            assert p.candidates == len(t) * 3 * inp.nq ** 2 * inp.nb ** 3
+        assert np.array_equal(c, cs) and np.array_equal(g, gs) and np.array_equal(w, ws)
+
+
+def test_paths_agree(fp):
+    """fused and split evaluate the same processes: identical counts, rates equal to rounding order."""
+    inp = fp_inputs.make_tiny("diamond", mesh=(4, 4, 4))
+    t = inp.targets4[24:48]
+    res = []
+    for path in PATHS(fp) + (fp.FP_PATH_SPLIT_SERIAL, fp.FP_PATH_AUTO):
+        with fp.Context.from_inputs(inp, scratch_bytes=128 << 20) as ctx:
+            ctx.set_path(path)
+            res.append(ctx.rates4(t) + ctx.rates3(inp.targets3))
+    for r in res[1:]:
+        for a, b in zip(res[0], r):
+            if a.dtype.kind == "i":
+                assert np.array_equal(a, b)
+            else:
+                assert np.allclose(a, b, rtol=1e-12, atol=1e-13 * np.abs(a).max())
+    assert all(np.array_equal(a, b) for a, b in zip(res[1], res[2]))   # overlap does not change the split path's bits
 
 
 def test_run_to_run_determinism(fp):
