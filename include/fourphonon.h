@@ -138,14 +138,18 @@ int fp_list4(fp_ctx *ctx, int32_t target, int32_t channel, int32_t qp, int32_t *
              void *stream);
 
 /* Execution path of fp_rates3 / fp_rates4 (same results bit for bit in counts, within rounding order in rates):
- *   FP_PATH_SPLIT  enumerator kernel -> process lists in the scratch region -> evaluator kernel (Algorithms 3 and 4,
- *                  PAPER.md:259-352, both on the device), chunks of rows sized to the scratch;
+ *   FP_PATH_SPLIT_SERIAL  enumerator kernel (pre-filter, pinned FP64 decision, weights) -> process lists in half of the
+ *                  scratch region -> evaluator kernel (|V|^2, row sums): Algorithms 3 and 4, both on
+ *                  the device, over chunks of rows sized to the scratch, back to back on the caller's stream;
+ *   FP_PATH_SPLIT  the same with two list buffers and a second (library-owned, high-priority) stream: the enumerator of
+ *                  chunk k+1 runs beside the evaluator of chunk k;
  *   FP_PATH_FUSED  one kernel per chunk of targets, lists in shared memory only (needs 20 bytes of scratch per row);
- *   FP_PATH_AUTO   (default) split when the scratch holds the lists of at least a few hundred rows, else fused.     */
+ *   FP_PATH_AUTO   (default) SPLIT_SERIAL when half of the scratch holds the lists of at least 256 rows (16 bytes x
+ *                  every candidate of a row), else FUSED.                                                            */
 #define FP_PATH_AUTO  0
 #define FP_PATH_FUSED 1
 #define FP_PATH_SPLIT 2
-#define FP_PATH_SPLIT_SERIAL 3   /* split without the two-stream overlap of enumerator and evaluator (for measurement) */
+#define FP_PATH_SPLIT_SERIAL 3
 int fp_set_path(fp_ctx *ctx, int path);
 
 /* Profiling of the library's own kernels (off by default; adds two cudaEventRecord per launch).                     */

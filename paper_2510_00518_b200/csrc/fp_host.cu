@@ -429,12 +429,15 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
     // ---- path: split (lists in the scratch) when half of the scratch holds two list buffers of a few hundred rows ------
     const int64_t capw = enum_slot_entries(d);
     const size_t row_list_bytes = (size_t)enum_warps_per_row() * ((size_t)capw * sizeof(ListEnt) + sizeof(uint32_t));
-    int64_t chunk_rows = (int64_t)std::min<size_t>((scratch_all / 2) / (2 * row_list_bytes), (size_t)1 << 20);
+    // FP_PATH_SPLIT runs the enumerator of chunk k+1 beside the evaluator of chunk k (two list buffers, two streams);
+    // FP_PATH_SPLIT_SERIAL -- what FP_PATH_AUTO picks -- runs them back to back through one buffer of twice the rows.
+    const bool overlap = ctx->path == FP_PATH_SPLIT;
+    const int nbuf = overlap ? 2 : 1;
+    int64_t chunk_rows = (int64_t)std::min<size_t>((scratch_all / 2) / (nbuf * row_list_bytes), (size_t)1 << 20);
     const int64_t rows_wanted = std::min<int64_t>(nt * nch * rows_per_unit, 256);
     bool split = ctx->path == FP_PATH_SPLIT || ctx->path == FP_PATH_SPLIT_SERIAL ||
                  (ctx->path == FP_PATH_AUTO && chunk_rows >= rows_wanted);
     if (split && chunk_rows < 1) return fail(ctx, FP_ENOMEM, "workspace scratch too small for the process lists of one row");
-    const bool overlap = split && ctx->path != FP_PATH_SPLIT_SERIAL;
     if (split && !ctx->side) {
         int prio_lo = 0, prio_hi = 0;                                // enumerator CTAs take freed SM slots first: they need
         CU(cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));    // few registers and keep the evaluator fed
@@ -444,7 +447,7 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
             CU(cudaEventCreateWithFlags(&ctx->ev_eval[i], cudaEventDisableTiming));
         }
     }
-    const size_t scratch = split ? scratch_all - 2 * (size_t)chunk_rows * row_list_bytes - 4096 : scratch_all;
+    const size_t scratch = split ? scratch_all - nbuf * (size_t)chunk_rows * row_list_bytes - 4096 : scratch_all;
     const size_t pre_per_target = (order == 3 ? (size_t)f.nblk * 9 : (size_t)f.n * 27) * sizeof(double2);
     const size_t per_target = pre_per_target + (size_t)rows_per_target * (4 + 16) + (size_t)nch * 24 + 4 + 64;
     const size_t fixed = 16 * 1024;
@@ -486,7 +489,7 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
             // chunks of rows through two list buffers: the enumerator of chunk k+1 (side stream) runs beside the evaluator
             // of chunk k (caller's stream); buffer b is rewritten only after the evaluator that read it has finished
             ListEnt *lists[2]; uint32_t *wcnt[2];
-            for (int b = 0; b < 2; b++) {
+            for (int b = 0; b < nbuf; b++) {
                 lists[b] = sc.take<ListEnt>((size_t)chunk_rows * enum_warps_per_row() * capw);
                 wcnt[b] = sc.take<uint32_t>((size_t)chunk_rows * enum_warps_per_row());
                 if (!lists[b] || !wcnt[b]) return fail(ctx, FP_ENOMEM, "scratch (process lists)");
@@ -499,7 +502,7 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
             int k = 0;
             for (int64_t r0 = 0; r0 < nrows; r0 += chunk_rows, k++) {
                 const int64_t nr = std::min(chunk_rows, nrows - r0);
-                const int b = k & 1;
+                const int b = overlap ? (k & 1) : 0;
                 RowArgs rc = ra; rc.row0 = r0;
                 if (overlap && k >= 2) CU(cudaStreamWaitEvent(es, ctx->ev_eval[b], 0));
                 { ProfScope p(ctx, CAT_ENUM, es);

@@ -35,7 +35,8 @@ struct FpDev {
     double wmin, wmax;
     const ModeRec *rec;           // N*nb
     const float4 *recf;           // N*nb  {omega, B1.v, B2.v, B3.v} rounded to FP32; omega = NaN marks a zero mode
-    const float2 *recn;           // N*nb  {omega (NaN for zero modes), n'} stage 1: admit iff |Delta_f| <= n'_a + n'_b
+    const float2 *recn;           // nb*N, branch-major [j][iq]: {omega (NaN for zero modes), n'}; stage 1 admits iff
+                                  // |Delta_f| <= n'_a + n'_b
     const double *occ;            // N*nb  f_lambda = 1/expm1(hbar omega/kB T)
     const double2 *evec;          // N*nb*nb mass-scaled eigenvectors e~ = e/sqrt(m)
     const double2 *evecc;         // N*nb*nb conj(e~): the conjugations of step 6 are table choices, not arithmetic

@@ -36,7 +36,9 @@ __global__ void k_tables(FpDev d, const double *omega, const double *eig, const 
         // stage 1 record: n' >= cs |u| + slack, rounded up (cs = ncut scale/sqrt(6), or n' = ncut sigma_const/2 + slack)
         const double un = sqrt(u0 * u0 + u1 * u1 + u2 * u2);
         const double nn = (d.sigma_const > 0.0 ? d.pfCs : d.pfCs * un) * (1.0 + 1e-6) + d.pfSlack;
-        recn[m] = make_float2(wf, isinf(d.pfCs) ? CUDART_INF_F : __double2float_ru(nn));   // ncut = inf: admit everything
+        // branch-major (recn[j*N + iq]): the 32 lanes of a stage-1 step read 32 consecutive q-points of one branch
+        recn[(m % d.nb) * (int64_t)d.N + m / d.nb] =
+            make_float2(wf, isinf(d.pfCs) ? CUDART_INF_F : __double2float_ru(nn));           // ncut = inf: admit everything
         atomicMax(maxima, (unsigned long long)__double_as_longlong(w));            // non-negative doubles order as integers
         atomicMax(maxima + 1, (unsigned long long)__double_as_longlong(un));
     }

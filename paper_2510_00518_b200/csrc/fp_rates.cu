@@ -220,6 +220,38 @@ __device__ __forceinline__ double2 contract_process(const FpDev &d, const BlkSme
 #endif
 
 
+// Two processes per lane against one pass over the row's blocks: every Mhat_b read from shared memory feeds 2 x 13
+// complex MACs, and the two dependency chains interleave (NAT > 0 only).
+template <int NAT>
+__device__ __forceinline__ void contract_process2(const FpDev &d, const BlkSmem &bs, const double2 *A0, const double2 *B0,
+                                                  int3 q0, const double2 *A1, const double2 *B1, int3 q1, double2 &V0,
+                                                  double2 &V1) {
+    V0 = make_double2(0.0, 0.0); V1 = make_double2(0.0, 0.0);
+#pragma unroll
+    for (int a = 0; a < NAT; a++)
+#pragma unroll
+        for (int c = 0; c < NAT; c++) {
+            const int b1 = bs.seg[a * NAT + c + 1];
+            for (int b = bs.seg[a * NAT + c]; b < b1; b++) {
+                const int4 m = bs.meta[b];
+                const double2 p0 = bs.ph[phase_idx(d, q0, m.y, m.z, m.w)], p1 = bs.ph[phase_idx(d, q1, m.y, m.z, m.w)];
+                const double2 *M = bs.M + 9 * b;
+                double2 u0 = make_double2(0.0, 0.0), u1 = make_double2(0.0, 0.0);
+#pragma unroll
+                for (int y = 0; y < 3; y++) {
+                    double2 t0 = make_double2(0.0, 0.0), t1 = make_double2(0.0, 0.0);
+#pragma unroll
+                    for (int x = 0; x < 3; x++) {
+                        const double2 mm = M[3 * x + y];
+                        cfma(t0, mm, A0[3 * a + x]); cfma(t1, mm, A1[3 * a + x]);
+                    }
+                    cfma(u0, t0, B0[3 * c + y]); cfma(u1, t1, B1[3 * c + y]);
+                }
+                cfma(V0, u0, p0); cfma(V1, u1, p1);
+            }
+        }
+}
+
 // ---------------------------------------------------------------------------------------------------------------------
 // a2/a3 + a5/a6 + a7: fused enumerate -> shared-memory queue -> evaluate
 // ---------------------------------------------------------------------------------------------------------------------
@@ -379,18 +411,18 @@ __device__ __forceinline__ int stage1_step(const FpDev &d, const Row &row, float
     const bool inq = qx < d.N;
     const int qs = inq ? qx : 0;
     const int ql = q_index(d, q_add(d, row.qb, row.s2, unpack_qc(d.qc[qs])));
-    const float2 *pa = d.recn + (size_t)qs * d.nb + ja0, *pb = d.recn + (size_t)ql * d.nb + jb0;
+    const float2 *pa = d.recn + (size_t)ja0 * d.N + qs, *pb = d.recn + (size_t)jb0 * d.N + ql;   // branch-major table
     float lo[TILE], hi[TILE];
 #pragma unroll
     for (int i = 0; i < TILE; i++) {
-        const float2 A = __ldg(pa + i);                               // omega_f = NaN for zero modes: never admitted
+        const float2 A = __ldg(pa + (size_t)i * d.N);                 // omega_f = NaN for zero modes: never admitted
         const float ba = inq ? (row.s2 > 0 ? basef + A.x : basef - A.x) : fnan;
         lo[i] = ba - A.y; hi[i] = ba + A.y;
     }
     uint64_t mask = 0;
 #pragma unroll
     for (int k = 0; k < TILE; k++) {
-        const float2 B = __ldg(pb + k);
+        const float2 B = __ldg(pb + (size_t)k * d.N);
         const float bl = B.x - B.y, bh = B.x + B.y;
 #pragma unroll
         for (int i = 0; i < TILE; i++)
@@ -607,8 +639,14 @@ __global__ void __launch_bounds__(RT, 8) k_enum(FpDev d, RowArgs ra, int64_t cap
 // Evaluator: |V|^2 of every listed process (level-2 contraction) and the row sums.  Every entry is an allowed process,
 // so the row count is the list length; the row factors of the weight (1/omega[omega'], occupation of lambda') multiply
 // the sums once.
+#ifndef FP_EVAL_PPL
+#define FP_EVAL_PPL 2                         // processes per lane of k_eval (NAT > 0): each Mhat read feeds two processes
+#endif
+#ifndef FP_EVAL_MINB
+#define FP_EVAL_MINB (FP_EVAL_PPL == 2 ? 3 : FP_MINB)
+#endif
 template <int ORDER, int NAT>
-__global__ void __launch_bounds__(RT, FP_MINB) k_eval(FpDev d, IfcDev f, RowArgs ra, const double2 *pre, int64_t capw,
+__global__ void __launch_bounds__(RT, FP_EVAL_MINB) k_eval(FpDev d, IfcDev f, RowArgs ra, const double2 *pre, int64_t capw,
                                                       const ListEnt *lists, const uint32_t *wcnt, double2 *partial,
                                                       uint32_t *counts) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -636,6 +674,27 @@ __global__ void __launch_bounds__(RT, FP_MINB) k_eval(FpDev d, IfcDev f, RowArgs
         return e;
     };
     double sG = 0.0, sW = 0.0;
+#if FP_EVAL_PPL == 2
+    if constexpr (NAT > 0 && FP_BLK_FORM == 0) {
+        for (unsigned base = warp * 64; base < total; base += 2 * RT) {   // 64 processes per warp pass, two per lane
+            const bool act0 = base + lane < total, act1 = base + 32 + lane < total;
+            const ListEnt e0 = fetch(act0 ? base + lane : base), e1 = fetch(act1 ? base + 32 + lane : base);
+            const int qx0 = (int)(e0.x >> 6), qx1 = (int)(e1.x >> 6);
+            const double2 *eA0 = (row.s2 > 0 ? d.evec : d.evecc) + ((size_t)qx0 * d.nb + (e0.x & 63u)) * d.nb;
+            const double2 *eA1 = (row.s2 > 0 ? d.evec : d.evecc) + ((size_t)qx1 * d.nb + (e1.x & 63u)) * d.nb;
+            const double2 *eB0 = d.evecc + ((size_t)(e0.y >> 6) * d.nb + (e0.y & 63u)) * d.nb;
+            const double2 *eB1 = d.evecc + ((size_t)(e1.y >> 6) * d.nb + (e1.y & 63u)) * d.nb;
+            const int3 xc0 = unpack_qc(__ldg(d.qc + qx0)), xc1 = unpack_qc(__ldg(d.qc + qx1));
+            double2 A0[3 * (NAT > 0 ? NAT : 1)], B0[3 * (NAT > 0 ? NAT : 1)], A1[3 * (NAT > 0 ? NAT : 1)], B1[3 * (NAT > 0 ? NAT : 1)];
+#pragma unroll
+            for (int c = 0; c < 3 * NAT; c++) { A0[c] = __ldg(eA0 + c); B0[c] = __ldg(eB0 + c); A1[c] = __ldg(eA1 + c); B1[c] = __ldg(eB1 + c); }
+            double2 V0, V1;
+            contract_process2<NAT>(d, bs, A0, B0, premul(d, xc0), A1, B1, premul(d, xc1), V0, V1);
+            if (act0) { sW += e0.w; sG = fma(e0.w, V0.x * V0.x + V0.y * V0.y, sG); }
+            if (act1) { sW += e1.w; sG = fma(e1.w, V1.x * V1.x + V1.y * V1.y, sG); }
+        }
+    } else
+#endif
     for (unsigned base = warp * 32; base < total; base += RT) {       // batch b of the row goes to warp b mod RW
         const bool act = base + lane < total;
         const ListEnt e = fetch(act ? base + lane : base);

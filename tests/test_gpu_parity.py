@@ -306,3 +306,46 @@ def test_kappa_matches_oracle(fp):
     ok = orc.kappa(gt)
     assert np.abs(k - ok).max() <= RTOL * np.abs(ok).max()
     assert np.allclose(k, k.T, rtol=1e-12, atol=1e-12 * np.abs(k).max())    # symmetric by construction
+
+
+# ---- BASELINE.json's full sizes, sampled: the oracle evaluates a seeded sample of targets (and a q' range for 4ph) -------
+def _sample(targets, n, seed, always=()):
+    rng = np.random.default_rng(seed)
+    pick = set(int(x) for x in rng.choice(np.asarray(targets), n, replace=False)) | set(int(x) for x in always)
+    return np.array(sorted(pick), dtype=np.int32)
+
+
+FULL_SCRATCH = 4 << 30
+
+
+def test_full_size_config1_3ph_sampled_modes(fp):
+    """config 1 (= the 3ph leg of config 3): 16x16x16, 24 of the 24,576 target modes incl. a Gamma acoustic mode."""
+    inp = fp_inputs.make_config(1)["main"]
+    t = _sample(inp.targets3, 23, 11, always=(0, 5, 24575))
+    g, c = check3(fp, inp, t, scratch_bytes=FULL_SCRATCH)
+    assert np.all(c[t == 0] == 0) and c.sum() > 100000
+
+
+def test_full_size_config2_4ph_sampled(fp):
+    """config 2: 8x8x8, three of the 192 targets over a q' range of 8 of the 512 points, all three channels."""
+    inp = fp_inputs.make_config(2)["main"]
+    t = np.ascontiguousarray(inp.targets4[[0, 77, 191]])
+    g, c = check4(fp, inp, t, qp=(37, 45), scratch_bytes=FULL_SCRATCH)
+    assert c.sum() > 100000
+
+
+def test_full_size_config3_4ph_sampled(fp):
+    """config 3: 16x16x16, two of the 96 targets (one acoustic, one optical branch) over q' in [1000, 1003)."""
+    inp = fp_inputs.make_config(3)["main"]
+    t = np.ascontiguousarray(inp.targets4[[1, 53]])
+    g, c = check4(fp, inp, t, qp=(1000, 1003), scratch_bytes=FULL_SCRATCH)
+    assert c.sum() > 100000
+
+
+def test_full_size_config4_sampled(fp):
+    """config 4 (8 atoms, 24 branches, generic kernels): 3ph at 12x12x12 on four modes, 4ph at 6x6x6 on one target x one q'."""
+    jobs = fp_inputs.make_config(4)
+    j3, j4 = jobs["3ph"], jobs["4ph"]
+    check3(fp, j3, _sample(j3.targets3, 3, 12, always=(7,)), scratch_bytes=FULL_SCRATCH)
+    g, c = check4(fp, j4, np.ascontiguousarray(j4.targets4[[29]]), qp=(17, 18), scratch_bytes=FULL_SCRATCH)
+    assert c.sum() > 10000
