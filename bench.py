@@ -28,6 +28,10 @@ if str(ROOT) not in sys.path:
 METRIC = "4ph processes/s (FP64)"
 UNIT = "processes/s"
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12     # 148 SMs x 64 FP64 FMA/clk/SM x 2 flop x 1965 MHz
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed ncu --set full
+# captures (profiles/r1c_summary.md); keyed by (config, path).  None = not captured for that configuration.
+NCU_DRAM_BYTES_PER_LAUNCH = {(3, "split"): 569.7e6}   # k_eval<4,2>, a 10,922-row launch of config 3: 563.8 MB read (the
+#                                                        process list k_enum wrote) + 5.9 MB written
 
 
 def workload(cfg: int):
@@ -151,7 +155,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--impl", default="b200")
-    ap.add_argument("--scratch-gb", type=float, default=16.0)
+    ap.add_argument("--scratch-gb", type=float, default=48.0,
+                    help="per-context scratch: half of it holds the process lists of the split path (DESIGN.md §5.2)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--path", choices=["auto", "fused", "split", "split-serial"], default="auto",
                     help="execution path of fp_rates3/4 (fp_set_path); auto = split when the scratch holds the lists")
@@ -283,10 +288,17 @@ def main():
         ctx.profile_enable(False)
     dom = max(kern, key=lambda k: kern[k][0])
     ms_c, n_c = kern["rates"]
+    ms_en, n_en = kern["enum"]
+    split = n_en > 0
     achieved = flops / (ms_c * 1e-3) / 1e12 if ms_c > 0 else 0.0
     probe = fp.fp_probe_fp64_tflops()
-    roofline = {"bound": "alu", "kernel": "k_rates (fused enumerate + V3/V4 contraction + weights)", "achieved": achieved,
-                "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS, "traffic": None,
+    kname = ("k_eval (V3/V4 level-2 contraction + row sums over the process lists; the enumerator k_enum is timed "
+             "separately, see kernel_ms_per_step)") if split else "k_rates (fused enumerate + V3/V4 contraction + weights)"
+    traffic = NCU_DRAM_BYTES_PER_LAUNCH.get((args.config, "split" if split else "fused"))
+    roofline = {"bound": "alu", "kernel": kname, "achieved": achieved,
+                "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS, "traffic": traffic,
+                "traffic_source": "profiles/r1c_summary.md (ncu --set full, dram bytes read + written, one launch)"
+                                  if traffic is not None else None,
                 "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (MEASURED_PEAKS.json has no FP64 "
                                f"entry); DFMA probe on this GPU measured {probe:.2f} TFLOP/s",
                 "flops_model": "allowed processes x nblk x 13 complex MAC x 8 flop (DESIGN.md §6); enumeration not counted",
@@ -295,7 +307,8 @@ def main():
                 "kernel_ms_per_step": {k: round(v[0], 3) for k, v in kern.items()},
                 "rows_per_step": rows, "candidates_per_step": cands, "prefiltered_per_step": pref,
                 "processes_per_step": procs,
-                "candidates_per_s_in_k_rates": cands / (ms_c * 1e-3) if ms_c > 0 else 0.0}
+                "candidates_per_s_in_enumerator": cands / ((ms_en if split else ms_c) * 1e-3) if ms_c > 0 else 0.0,
+                "path": "split" if split else "fused"}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
