@@ -36,11 +36,33 @@ __device__ __forceinline__ int phase_idx(const FpDev &d, int3 qm, int n1, int n2
 }
 __device__ __forceinline__ int3 premul(const FpDev &d, int3 c) { return make_int3(c.x * d.m1, c.y * d.m2, c.z * d.m3); }
 
+#ifndef FP_LDG256
+#define FP_LDG256 1     // gathers of 32-byte aligned records go through one 256-bit load per 32-byte sector (LDG.E.256, sm_100)
+#endif
+// 32 bytes at a 32-byte aligned address through the read-only path: one request per sector instead of two
+__device__ __forceinline__ void ldg256(const void *p, double2 &lo, double2 &hi) {
+#if FP_LDG256
+    asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(lo.x), "=d"(lo.y), "=d"(hi.x), "=d"(hi.y) : "l"(p));
+#else
+    lo = __ldg(reinterpret_cast<const double2 *>(p)); hi = __ldg(reinterpret_cast<const double2 *>(p) + 1);
+#endif
+}
 __device__ __forceinline__ ModeRec load_rec(const ModeRec *p) {
-    const double2 *q = reinterpret_cast<const double2 *>(p);
-    double2 a = __ldg(q), b = __ldg(q + 1);
+    double2 a, b;
+    ldg256(p, a, b);
     ModeRec r; r.omega = a.x; r.vx = a.y; r.vy = b.x; r.vz = b.y;
     return r;
+}
+// NC complex components of one eigenvector (NC even: the vector is a whole number of 32-byte sectors)
+template <int NC>
+__device__ __forceinline__ void load_evec(const double2 *__restrict__ e, double2 *dst) {
+    if constexpr (NC % 2 == 0) {
+#pragma unroll
+        for (int c = 0; c < NC; c += 2) ldg256(e + c, dst[c], dst[c + 1]);
+    } else {
+#pragma unroll
+        for (int c = 0; c < NC; c++) dst[c] = __ldg(e + c);
+    }
 }
 
 struct Row {

@@ -286,15 +286,13 @@ __device__ __forceinline__ void eval_process(const FpDev &d, const BlkSmem &bs, 
     const int3 xc = unpack_qc(__ldg(d.qc + qx));
     double2 A[3 * (NAT > 0 ? NAT : 1)], Bc[3 * (NAT > 0 ? NAT : 1)];
     if constexpr (NAT > 0) {
-#pragma unroll
-        for (int c = 0; c < 3 * NAT; c++) A[c] = __ldg(eA + c);
+        load_evec<3 * NAT>(eA, A);
 #if FP_BLK_FORM == 1 && FP_LATE_B
 #if !FP_EVAL_PF
         prefetch_l1(eB); prefetch_l1(eB + 3 * NAT - 1);
 #endif
 #else
-#pragma unroll
-        for (int c = 0; c < 3 * NAT; c++) Bc[c] = __ldg(eB + c);
+        load_evec<3 * NAT>(eB, Bc);
 #endif
     }
     // the decision, in the pinned arithmetic
@@ -686,8 +684,7 @@ __global__ void __launch_bounds__(RT, FP_EVAL_MINB) k_eval(FpDev d, IfcDev f, Ro
             const double2 *eB1 = d.evecc + ((size_t)(e1.y >> 6) * d.nb + (e1.y & 63u)) * d.nb;
             const int3 xc0 = unpack_qc(__ldg(d.qc + qx0)), xc1 = unpack_qc(__ldg(d.qc + qx1));
             double2 A0[3 * (NAT > 0 ? NAT : 1)], B0[3 * (NAT > 0 ? NAT : 1)], A1[3 * (NAT > 0 ? NAT : 1)], B1[3 * (NAT > 0 ? NAT : 1)];
-#pragma unroll
-            for (int c = 0; c < 3 * NAT; c++) { A0[c] = __ldg(eA0 + c); B0[c] = __ldg(eB0 + c); A1[c] = __ldg(eA1 + c); B1[c] = __ldg(eB1 + c); }
+            load_evec<3 * NAT>(eA0, A0); load_evec<3 * NAT>(eB0, B0); load_evec<3 * NAT>(eA1, A1); load_evec<3 * NAT>(eB1, B1);
             double2 V0, V1;
             contract_process2<NAT>(d, bs, A0, B0, premul(d, xc0), A1, B1, premul(d, xc1), V0, V1);
             if (act0) { sW += e0.w; sG = fma(e0.w, V0.x * V0.x + V0.y * V0.y, sG); }
@@ -704,8 +701,7 @@ __global__ void __launch_bounds__(RT, FP_EVAL_MINB) k_eval(FpDev d, IfcDev f, Ro
         const int3 xc = unpack_qc(__ldg(d.qc + qx));
         double2 A[3 * (NAT > 0 ? NAT : 1)], Bc[3 * (NAT > 0 ? NAT : 1)];
         if constexpr (NAT > 0) {
-#pragma unroll
-            for (int c = 0; c < 3 * NAT; c++) { A[c] = __ldg(eA + c); Bc[c] = __ldg(eB + c); }
+            load_evec<3 * NAT>(eA, A); load_evec<3 * NAT>(eB, Bc);
         }
         const double2 V = contract_process<NAT>(d, bs, eA, eB, A, Bc, premul(d, xc));
         if (act) {
