@@ -86,6 +86,7 @@ typedef struct {
     double  rates_flops;    /* FP64 flops of the per-process contraction (analytic model)             */
     double  ms_enum;        /* split path: summed durations of the enumerator kernel (ms_rates is then the evaluator) */
     int64_t n_enum;
+    int64_t list_overflows; /* split path: (row, warp) list slots that filled up (their super-chunk was redone fused) */
 } fp_profile;
 
 /* Bytes of workspace fp_setup needs for its resident tables plus `scratch_bytes` of per-call scratch (per-target

@@ -74,7 +74,7 @@ class _Profile(C.Structure):
     _fields_ = [(n, C.c_double) for n in ("ms_precontract", "ms_rates", "ms_reduce")] + \
                [(n, C.c_int64) for n in ("n_precontract", "n_rates", "n_reduce", "rows", "candidates", "prefiltered",
                                          "processes")] + [("rates_flops", C.c_double), ("ms_enum", C.c_double),
-                                                          ("n_enum", C.c_int64)]
+                                                          ("n_enum", C.c_int64), ("list_overflows", C.c_int64)]
 
 
 @dataclass
@@ -92,6 +92,7 @@ class Profile:
     rates_flops: float
     ms_enum: float = 0.0
     n_enum: int = 0
+    list_overflows: int = 0
 
     @property
     def launches(self) -> int:

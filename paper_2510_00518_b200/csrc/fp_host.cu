@@ -427,7 +427,11 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
     // ---- scratch budget: per-target arrays for a super-chunk of targets ------------------------------------------------
     const size_t scratch_all = ctx->ws_bytes - ctx->resident;
     // ---- path: split (lists in the scratch) when half of the scratch holds two list buffers of a few hundred rows ------
-    const int64_t capw = enum_slot_entries(d);
+    // list slot of one (row, warp): a quarter of what can never overflow (but at least 2048 entries); a slot that fills
+    // up is flagged by k_enum and the super-chunk is redone through the fused kernel (never seen on the configs: the
+    // filter admits 2-5 % of the candidates)
+    const int64_t capw_all = enum_slot_entries(d);
+    const int64_t capw = std::min(capw_all, std::max<int64_t>(((capw_all / 4) + 31) & ~(int64_t)31, 2048));
     const size_t row_list_bytes = (size_t)enum_warps_per_row() * ((size_t)capw * sizeof(ListEnt) + sizeof(uint32_t));
     // FP_PATH_SPLIT runs the enumerator of chunk k+1 beside the evaluator of chunk k (two list buffers, two streams);
     // FP_PATH_SPLIT_SERIAL -- what FP_PATH_AUTO picks -- runs them back to back through one buffer of twice the rows.
@@ -471,14 +475,15 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
         double2 *pre = sc.take<double2>(nts * (pre_per_target / sizeof(double2)));
         uint32_t *cnt = sc.take<uint32_t>(nrows);
         double2 *partial = sc.take<double2>(nrows);
-        unsigned long long *stat = sc.take<unsigned long long>(1);
+        unsigned long long *stat = sc.take<unsigned long long>(2);    // [0] pre-filter survivors, [1] list overflows
         double *o_gamma = sc.take<double>(nts * nch), *o_wp = sc.take<double>(nts * nch);
         int64_t *o_cnt = sc.take<int64_t>(nts * nch);
         if (!pre || !cnt || !partial || !stat || !o_gamma || !o_wp || !o_cnt) return fail(ctx, FP_ENOMEM, "scratch");
 
         RowArgs ra; ra.targets = d_targets; ra.row0 = 0; ra.qp_begin = qp_begin; ra.nqp = (int)nqp;
         ra.prefiltered = ctx->profiling ? stat : nullptr;
-        if (ctx->profiling) CU(cudaMemsetAsync(stat, 0, sizeof(unsigned long long), st));
+        ra.overflow = reinterpret_cast<unsigned int *>(stat + 1);
+        CU(cudaMemsetAsync(stat, 0, 2 * sizeof(unsigned long long), st));
         { ProfScope p(ctx, CAT_PRE, st);
           if (order == 3) launch_pre3(d, f, d_targets, nts, pre, st); else launch_pre4(d, f, d_targets, nts, pre, st); }
         CU(cudaGetLastError());
@@ -514,6 +519,15 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
                 { ProfScope p(ctx, CAT_RATES, st);
                   CU(launch_eval(order, d, f, rc, nr, pre, capw, lists[b], wcnt[b], partial + r0, cnt + r0, st)); }
                 if (overlap) CU(cudaEventRecord(ctx->ev_eval[b], st));
+            }
+            unsigned long long novf = 0;
+            CU(cudaMemcpyAsync(&novf, stat + 1, sizeof(novf), cudaMemcpyDeviceToHost, st));
+            CU(cudaStreamSynchronize(st));
+            if (novf != 0) {                                         // some list slot filled up: redo with lists in shared memory
+                ctx->prof.list_overflows += (int64_t)novf;
+                if (ctx->profiling) CU(cudaMemsetAsync(stat, 0, sizeof(unsigned long long), st));
+                ProfScope p(ctx, CAT_RATES, st);
+                CU(launch_rates(order, d, f, ra, nrows, pre, partial, cnt, st));
             }
         }
         double *g_out = loc == FP_MEM_DEVICE ? gamma + t0 * nch : o_gamma;
@@ -597,7 +611,7 @@ static int list_driver(fp_ctx *ctx, int order, int32_t target, int32_t channel, 
     int64_t *offs = sc.take<int64_t>(nrows + 1), *bsums = sc.take<int64_t>(16);
     if (!d_t || !cnt || !offs || !bsums) return fail(ctx, FP_ENOMEM, "scratch");
     CU(cudaMemcpyAsync(d_t, &target, 4, cudaMemcpyHostToDevice, st));
-    RowArgs ra; ra.targets = d_t; ra.row0 = 0; ra.qp_begin = qp; ra.nqp = 1; ra.prefiltered = nullptr;
+    RowArgs ra; ra.targets = d_t; ra.row0 = 0; ra.qp_begin = qp; ra.nqp = 1; ra.prefiltered = nullptr; ra.overflow = nullptr;
     launch_count(order, d, ra, nrows, cnt, st);
     launch_scan(cnt, nrows, offs, bsums, st);
     std::vector<int64_t> ho(nrows + 1);

@@ -64,6 +64,8 @@ struct RowArgs {
     int64_t row0;                 // first row handled by this launch
     int qp_begin, nqp;            // 4ph only
     unsigned long long *prefiltered;   // nullable: += candidates admitted by the FP32 pre-filter (profiling)
+    unsigned int *overflow;       // split path: += 1 for every (row, warp) list slot that filled up (the driver then
+                                  // re-runs the super-chunk through the fused kernel)
 };
 
 // One allowed process of a row in the split path: both free legs and the row-independent part of its weight.
@@ -104,7 +106,7 @@ cudaError_t launch_rates(int order, const FpDev &d, const IfcDev &f, const RowAr
                          double2 *partial, uint32_t *counts, cudaStream_t st);
 size_t rates_smem_bytes(const FpDev &d, const IfcDev &f);
 // split path (fp_rates.cu): enumerator -> process lists in the scratch -> evaluator
-int64_t enum_slot_entries(const FpDev &d);        // entries of one (row, warp) list slot
+int64_t enum_slot_entries(const FpDev &d);        // entries of one (row, warp) list slot that can never overflow
 int enum_warps_per_row();
 cudaError_t launch_enum(int order, const FpDev &d, const RowArgs &ra, int64_t nrows, int64_t capw, ListEnt *lists,
                         uint32_t *wcnt, cudaStream_t st);

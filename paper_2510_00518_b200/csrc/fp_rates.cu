@@ -579,6 +579,7 @@ __global__ void __launch_bounds__(RT, 8) k_enum(FpDev d, RowArgs ra, int64_t cap
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const Row row = make_row<ORDER>(d, ra, ra.row0 + r);
     unsigned nout = 0, nadm = 0;
+    bool ovf = false;                                                 // the slot filled up: the row is redone by k_rates
     if (row.valid && !row_is_empty(d, row)) {                         // item 8: zero modes are never a leg
         ListEnt *out = lists + ((size_t)r * RW + warp) * (size_t)capw;
         uint32_t *pend = pendq + warp * PCAP;
@@ -617,17 +618,23 @@ __global__ void __launch_bounds__(RT, 8) k_enum(FpDev d, RowArgs ra, int64_t cap
                     w = occ * (exp(-(rr * rr)) * t * 0.56418958354775628695);   // 1/sqrt(pi)
                 }
                 const unsigned bal = __ballot_sync(0xffffffffu, ok);
-                if (ok) {
-                    ListEnt e; e.x = e2.x; e.y = e2.y; e.w = w;
-                    out[nout + __popc(bal & ((1u << lane) - 1u))] = e;
+                if (nout + __popc(bal) > (unsigned)capw) ovf = true;  // warp-uniform
+                else {
+                    if (ok) {
+                        ListEnt e; e.x = e2.x; e.y = e2.y; e.w = w;
+                        out[nout + __popc(bal & ((1u << lane) - 1u))] = e;
+                    }
+                    nout += __popc(bal);
                 }
-                nout += __popc(bal);
                 nadm += pass ? 1u : 0u;
             }
             __syncwarp();
         }
     }
-    if (lane == 0) wcnt[r * RW + warp] = nout;
+    if (lane == 0) {
+        wcnt[r * RW + warp] = ovf ? 0xffffffffu : nout;
+        if (ovf) atomicAdd(ra.overflow, 1u);
+    }
     if (ra.prefiltered) {                                             // profiling only: pre-filter survivors
         for (int o = 16; o > 0; o >>= 1) nadm += __shfl_down_sync(0xffffffffu, nadm, o);
         if (lane == 0 && nadm) atomicAdd(ra.prefiltered, (unsigned long long)nadm);
@@ -651,7 +658,9 @@ __global__ void __launch_bounds__(RT, FP_EVAL_MINB) k_eval(FpDev d, IfcDev f, Ro
     __shared__ double red[32];
     const int64_t r = blockIdx.x;
     const uint4 wc = __ldg(reinterpret_cast<const uint4 *>(wcnt) + r);
-    const unsigned p1 = wc.x, p2 = p1 + wc.y, p3 = p2 + wc.z, total = p3 + wc.w;
+    const bool ovf = (wc.x & wc.y & wc.z & wc.w) == 0xffffffffu || wc.x == 0xffffffffu || wc.y == 0xffffffffu ||
+                     wc.z == 0xffffffffu || wc.w == 0xffffffffu;      // a slot of the row filled up: redone by k_rates
+    const unsigned p1 = wc.x, p2 = p1 + wc.y, p3 = p2 + wc.z, total = ovf ? 0u : p3 + wc.w;
     if (total == 0) {
         if (threadIdx.x == 0) { partial[r] = make_double2(0.0, 0.0); counts[r] = 0; }
         return;

@@ -349,3 +349,27 @@ def test_full_size_config4_sampled(fp):
     check3(fp, j3, _sample(j3.targets3, 3, 12, always=(7,)), scratch_bytes=FULL_SCRATCH)
     g, c = check4(fp, j4, np.ascontiguousarray(j4.targets4[[29]]), qp=(17, 18), scratch_bytes=FULL_SCRATCH)
     assert c.sum() > 10000
+
+
+def test_list_overflow_falls_back_to_fused(fp):
+    """With the filter disabled every candidate is allowed, so the split path's list slots (a quarter of the candidates,
+    at least 2048 entries) fill up on an 8x8x8 mesh: k_enum flags them and the driver redoes the super-chunk fused."""
+    inp = fp_inputs.make_tiny("diamond", mesh=(8, 8, 8))
+    t = np.ascontiguousarray(inp.targets4[[100, 205]])
+    kw = dict(ncut=np.inf, sigma_const=5.0)
+    og, ow, oc = _oracle(inp, **kw).rates4(t, 5, 6)
+    with fp.Context.from_inputs(inp, scratch_bytes=256 << 20, **kw) as ctx:
+        ctx.set_path(fp.FP_PATH_SPLIT_SERIAL)
+        ctx.profile_enable(True)
+        g, w, c = ctx.rates4(t, 5, 6)
+        p = ctx.profile_get()
+    assert p.list_overflows > 0 and p.n_enum > 0
+    assert np.array_equal(c, oc)
+    assert_rates_close(g, og, "Gamma4 (overflow fallback)")
+    assert_rates_close(w, ow, "WP4 (overflow fallback)")
+    # the ordinary filter never comes near the slot size
+    with fp.Context.from_inputs(inp, scratch_bytes=256 << 20) as ctx:
+        ctx.set_path(fp.FP_PATH_SPLIT_SERIAL)
+        ctx.profile_enable(True)
+        ctx.rates4(t, 5, 6)
+        assert ctx.profile_get().list_overflows == 0
