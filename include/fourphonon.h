@@ -77,16 +77,16 @@ typedef struct {
 
 /* Device-time profile of the kernels launched since the last fp_profile_reset (CUDA events on the launch stream).   */
 typedef struct {
-    double  ms_precontract, ms_rates, ms_reduce;      /* summed launch durations, ms: per-target pre-contraction,     */
-    int64_t n_precontract, n_rates, n_reduce;         /* fused enumerate+evaluate kernel, per-mode reduction; launches */
-    int64_t rows;           /* rows ((target, channel[, lambda']) units, one CTA each) of the fused kernel               */
+    double  ms_precontract, ms_rates, ms_reduce;      /* summed launch durations, ms: per-target pre-contraction, the  */
+    int64_t n_precontract, n_rates, n_reduce;         /* evaluator (k_eval; fused: k_rates), per-mode reduction; launches */
+    int64_t rows;           /* rows ((target, channel[, lambda']) units, one CTA each per kernel)                        */
     int64_t candidates;     /* momentum-conserving candidates examined by the enumerator                            */
     int64_t prefiltered;    /* candidates admitted by the FP32 pre-filter (superset of the allowed ones)            */
     int64_t processes;      /* allowed processes (pinned FP64 decision) evaluated                                   */
     double  rates_flops;    /* FP64 flops of the per-process contraction (analytic model)             */
     double  ms_enum;        /* split path: summed durations of the enumerator kernel (ms_rates is then the evaluator) */
     int64_t n_enum;
-    int64_t list_overflows; /* split path: (row, warp) list slots that filled up (their super-chunk was redone fused) */
+    int64_t list_overflows; /* split path: (row, warp) list slots that filled up (their rows were redone fused)      */
 } fp_profile;
 
 /* Bytes of workspace fp_setup needs for its resident tables plus `scratch_bytes` of per-call scratch (per-target

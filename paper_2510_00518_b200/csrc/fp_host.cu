@@ -63,7 +63,7 @@ long gcdl(long a, long b) { while (b) { long t = a % b; a = b; b = t; } return a
 
 // Host-side analysis of an IFC list: group clusters into contraction blocks (atomA, atomB, dR) -- DESIGN.md §5.
 struct IfcHost {
-    int n = 0, nblk = 0, ncomp = 0, ngrp = 0;
+    int n = 0, nblk = 0, ncomp = 0;
     std::vector<int4> meta0, meta1, blk_meta;
     std::vector<double> phi;
     std::vector<int> blk_start, seg;
@@ -83,7 +83,7 @@ int analyse_ifc(const fp_ifc *f, int order, int nat, const int32_t mesh[3], IfcH
             if (at[m] < 0 || at[m] >= nat) { err = "IFC atom index out of range"; return FP_EINVAL; }
         const int32_t *RA = f->cells + (size_t)c * (order - 1) * 3 + (order - 3) * 3;   // leg A: j (3ph) / k (4ph)
         const int32_t *RB = RA + 3;                                                      // leg B: k (3ph) / l (4ph)
-        key[c] = Key(at[order - 2 + FP_BLK_FORM], at[order - 1 - FP_BLK_FORM], imod((long)RA[0] - RB[0], mesh[0]), imod((long)RA[1] - RB[1], mesh[1]),
+        key[c] = Key(at[order - 2], at[order - 1], imod((long)RA[0] - RB[0], mesh[0]), imod((long)RA[1] - RB[1], mesh[1]),
                      imod((long)RA[2] - RB[2], mesh[2]));
         blocks.emplace(key[c], 0);
     }
@@ -94,14 +94,12 @@ int analyse_ifc(const fp_ifc *f, int order, int nat, const int32_t mesh[3], IfcH
     for (auto &kv : blocks) {                                // std::map iterates sorted by (atomA, atomB, dR)
         kv.second = id;
         const Key &k = kv.first;
-        h.blk_meta[id] = make_int4(std::get<FP_BLK_FORM>(k) | (std::get<1 - FP_BLK_FORM>(k) << 16), std::get<2>(k), std::get<3>(k),
+        h.blk_meta[id] = make_int4(std::get<0>(k) | (std::get<1>(k) << 16), std::get<2>(k), std::get<3>(k),
                                    std::get<4>(k));           // {atomA | atomB << 16, dR}; key order = sort order
         h.seg[std::get<0>(k) * nat + std::get<1>(k) + 1]++;
         id++;
     }
     for (int i = 0; i < nat * nat; i++) h.seg[i + 1] += h.seg[i];
-    h.ngrp = 0;                                              // first-key groups with at least one block
-    for (int c = 0; c < nat; c++) h.ngrp += h.seg[(c + 1) * nat] > h.seg[c * nat];
     std::vector<int> order_idx(h.n);
     for (int c = 0; c < h.n; c++) order_idx[c] = c;
     std::stable_sort(order_idx.begin(), order_idx.end(), [&](int a, int b) { return blocks[key[a]] < blocks[key[b]]; });
@@ -164,7 +162,7 @@ int upload_ifc(fp_ctx *ctx, Bump &bump, const IfcHost &h, IfcDev &dv, cudaStream
     CU(cudaMemcpyAsync(bs, h.blk_start.data(), (h.nblk + 1) * sizeof(int), cudaMemcpyHostToDevice, st));
     CU(cudaMemcpyAsync(seg, h.seg.data(), (nat * nat + 1) * sizeof(int), cudaMemcpyHostToDevice, st));
     CU(cudaStreamSynchronize(st));                                   // host vectors go out of scope after setup
-    dv.n = h.n; dv.nblk = h.nblk; dv.ncomp = h.ncomp; dv.ngrp = h.ngrp;
+    dv.n = h.n; dv.nblk = h.nblk; dv.ncomp = h.ncomp;
     dv.cl_meta0 = m0; dv.cl_meta1 = m1; dv.phi = phi; dv.blk_start = bs; dv.blk_meta = bm; dv.seg = seg;
     return FP_OK;
 }
@@ -428,8 +426,8 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
     const size_t scratch_all = ctx->ws_bytes - ctx->resident;
     // ---- path: split (lists in the scratch) when half of the scratch holds two list buffers of a few hundred rows ------
     // list slot of one (row, warp): a quarter of what can never overflow (but at least 2048 entries); a slot that fills
-    // up is flagged by k_enum and the super-chunk is redone through the fused kernel (never seen on the configs: the
-    // filter admits 2-5 % of the candidates)
+    // up is flagged by k_enum and its row is redone through the fused kernel (rows of the many-branch config 4, where
+    // the +- channel admits 10 % and more of the candidates; never on the diamond configs)
     const int64_t capw_all = enum_slot_entries(d);
     const int64_t capw = std::min(capw_all, std::max<int64_t>(((capw_all / 4) + 31) & ~(int64_t)31, 2048));
     const size_t row_list_bytes = (size_t)enum_warps_per_row() * ((size_t)capw * sizeof(ListEnt) + sizeof(uint32_t));
@@ -489,7 +487,7 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
         CU(cudaGetLastError());
         if (!split) {
             ProfScope p(ctx, CAT_RATES, st);
-            CU(launch_rates(order, d, f, ra, nrows, pre, partial, cnt, st));
+            CU(launch_rates(order, d, f, ra, nrows, pre, partial, cnt, false, st));
         } else {
             // chunks of rows through two list buffers: the enumerator of chunk k+1 (side stream) runs beside the evaluator
             // of chunk k (caller's stream); buffer b is rewritten only after the evaluator that read it has finished
@@ -523,11 +521,11 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
             unsigned long long novf = 0;
             CU(cudaMemcpyAsync(&novf, stat + 1, sizeof(novf), cudaMemcpyDeviceToHost, st));
             CU(cudaStreamSynchronize(st));
-            if (novf != 0) {                                         // some list slot filled up: redo with lists in shared memory
-                ctx->prof.list_overflows += (int64_t)novf;
-                if (ctx->profiling) CU(cudaMemsetAsync(stat, 0, sizeof(unsigned long long), st));
+            if (novf != 0) {                                         // some list slots filled up: k_eval marked their rows in
+                ctx->prof.list_overflows += (int64_t)novf;           // cnt; redo those with the lists in shared memory
+                RowArgs rr = ra; rr.prefiltered = nullptr;
                 ProfScope p(ctx, CAT_RATES, st);
-                CU(launch_rates(order, d, f, ra, nrows, pre, partial, cnt, st));
+                CU(launch_rates(order, d, f, rr, nrows, pre, partial, cnt, true, st));
             }
         }
         double *g_out = loc == FP_MEM_DEVICE ? gamma + t0 * nch : o_gamma;
@@ -553,8 +551,7 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
             ctx->prof.processes += total;
             ctx->prof.prefiltered += (int64_t)hstat;
             ctx->prof.candidates += nrows * row_cands;
-            ctx->prof.rates_flops += (double)total * 8.0 *
-                                     (FP_BLK_FORM ? (double)f.nblk * 12.0 + (double)f.ngrp * 3.0 : (double)f.nblk * 13.0);
+            ctx->prof.rates_flops += (double)total * (double)f.nblk * 13.0 * 8.0;
         }
     }
     return FP_OK;

@@ -13,9 +13,6 @@
 
 #include "../../include/fourphonon.h"
 
-#ifndef FP_BLK_FORM
-#define FP_BLK_FORM 0         // 0: blocks sorted (atomA, atomB), V += phase*(t.Bc); 1: sorted (atomB, atomA), W_c += phase*t
-#endif
 #define FP_MAX_NB 64          // branch-mask width of the enumerator (natoms <= 21)
 #define FP_MAX_L 4096         // lcm of the mesh dimensions (1-D phase table in shared memory)
 
@@ -50,7 +47,6 @@ struct FpDev {
 // All cell offsets are stored reduced to [0,N_mu).
 struct IfcDev {
     int n, nblk, ncomp;           // clusters, blocks, 27 or 81
-    int ngrp;                     // atomB groups with at least one block (flop model of FP_BLK_FORM 1)
     const int4 *cl_meta0;         // n
     const int4 *cl_meta1;         // n (ORDER 4 only)
     const double *phi;            // n*ncomp, block-sorted
@@ -65,7 +61,7 @@ struct RowArgs {
     int qp_begin, nqp;            // 4ph only
     unsigned long long *prefiltered;   // nullable: += candidates admitted by the FP32 pre-filter (profiling)
     unsigned int *overflow;       // split path: += 1 for every (row, warp) list slot that filled up (the driver then
-                                  // re-runs the super-chunk through the fused kernel)
+                                  // re-runs those rows through the fused kernel)
 };
 
 // One allowed process of a row in the split path: both free legs and the row-independent part of its weight.
@@ -102,8 +98,9 @@ void launch_tables(const FpDev &d, const double *omega, const double *eig, const
 // fused rate kernel (fp_rates.cu)
 void launch_pre3(const FpDev &d, const IfcDev &f, const int32_t *targets, int64_t nt, double2 *mhat, cudaStream_t st);
 void launch_pre4(const FpDev &d, const IfcDev &f, const int32_t *targets, int64_t nt, double2 *t0, cudaStream_t st);
+// only_flagged: redo pass of the split path -- only rows with counts[r] == 0xffffffff (a list slot filled up) are computed
 cudaError_t launch_rates(int order, const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const double2 *pre,
-                         double2 *partial, uint32_t *counts, cudaStream_t st);
+                         double2 *partial, uint32_t *counts, bool only_flagged, cudaStream_t st);
 size_t rates_smem_bytes(const FpDev &d, const IfcDev &f);
 // split path (fp_rates.cu): enumerator -> process lists in the scratch -> evaluator
 int64_t enum_slot_entries(const FpDev &d);        // entries of one (row, warp) list slot that can never overflow

@@ -1,19 +1,21 @@
-// fp_rates.cu -- the fused rate kernel of the FourPhonon hot path (SURVEY.md §8(a) rows a2/a3 + a5/a6 + a7) and the
+// fp_rates.cu -- the rate kernels of the FourPhonon hot path (SURVEY.md §8(a) rows a2/a3 + a5/a6 + a7) and the
 // per-target pre-contraction.
 //
 //   k_pre3/k_pre4  per-target level-0 contraction of the IFC list with the target eigenvector
-//   k_rates        one CTA per row (3ph: (target, channel); 4ph: (target, channel, lambda')).  Each warp enumerates its
-//                  share of the row's candidates (momentum modulo the mesh PAPER.md:155,288; energy window
-//                  PAPER.md:163,293), compacts the survivors into a warp-private queue in shared memory (ballot-free
-//                  ordered scan), and whenever 32 are queued evaluates them: exact window decision in the pinned FP64
-//                  arithmetic of SURVEY.md §8(c) step 3, matrix element (compute_Vp), Gaussian and
-//                  occupation weights, accumulation.  Nothing is written to global
-//                  memory but one partial sum and one count per row: the process lists of Algorithm 3
-//                   live and die in shared memory.
+//   split path (default): Algorithm 3 -> Algorithm 4 of the paper, both on the device
+//     k_enum       one CTA per row (3ph: (target, channel); 4ph: (target, channel, lambda')).  Each warp enumerates its
+//                  share of the row's candidates (momentum modulo the mesh PAPER.md:155,288), filters them with the
+//                  two-stage FP32 pre-filter, takes the window decision in the pinned FP64 arithmetic
+//                  of SURVEY.md §8(c) step 3, computes the row-independent part of the weight and
+//                  ballot-compacts the allowed processes into its list slot (16 bytes per process)
+//     k_eval       one CTA per row: matrix element of every listed process (compute_Vp), two processes
+//                  per lane against one pass over the row's contraction blocks, accumulation
+//   fused path (small scratch, or a list slot that filled up)
+//     k_rates      one CTA per row does all of the above; the process lists live and die in shared memory
 //
-// The window is decided twice.  A cheap FP32 pre-filter (table recf: omega and u = B v rounded to FP32) admits a
+// The window is decided twice.  A cheap FP32 pre-filter (tables recn / recf: omega and u = B v rounded to FP32) admits a
 // proven superset of the allowed candidates (error budget in DESIGN.md §5.2, constants pfK1/pfC2 from fp_setup); only
-// the ~5 % survivors pay for the pinned FP64 decision, which alone determines counts and rates.
+// the ~2.5 % survivors pay for the pinned FP64 decision, which alone determines counts and rates.
 //
 // Contraction algebra: with the momentum modulo, phi(-q_last,R) factorises, so per row
 //   V = sum_b phi(s2 qx, dR_b) sum_{xy} Mhat_b[x][y] A(atomA_b,x) conj(e~_B(atomB_b,y)),
@@ -83,18 +85,6 @@ struct BlkSmem {
     int *seg;          // nat*nat+1
 };
 
-#ifndef FP_BLK_UNROLL
-#define FP_BLK_UNROLL 1
-#endif
-#ifndef FP_LATE_B
-#define FP_LATE_B 0                           // FP_BLK_FORM 1: fetch the B eigenvector when its group closes (L1 hit)
-#endif
-#ifndef FP_EVAL_PF
-#define FP_EVAL_PF 0                          // k_eval prefetches the records and eigenvectors of the next batch into L1
-#endif
-constexpr int kBlkUnroll = FP_BLK_UNROLL;
-__device__ __forceinline__ void prefetch_l1(const void *p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
-#if FP_BLK_FORM == 0
 // One block: u = sum_y (sum_x M[x][y] A[x]) Bc[y];  V += u * phase          (13 complex MAC = 52 DFMA)
 __device__ __forceinline__ void block_term(const double2 *M, const double2 *A, const double2 *Bc, double2 ph, double2 &V) {
     double2 u = make_double2(0.0, 0.0);
@@ -123,7 +113,6 @@ __device__ __forceinline__ double2 contract_process(const FpDev &d, const BlkSme
 #pragma unroll
             for (int c = 0; c < NAT; c++) {
                 const int b1 = bs.seg[a * NAT + c + 1];
-#pragma unroll kBlkUnroll
                 for (int b = bs.seg[a * NAT + c]; b < b1; b++) {
                     const int4 m = bs.meta[b];
                     block_term(bs.M + 9 * b, A + 3 * a, Bc + 3 * c, bs.ph[phase_idx(d, qmx, m.y, m.z, m.w)], V);
@@ -141,7 +130,6 @@ __device__ __forceinline__ double2 contract_process(const FpDev &d, const BlkSme
                 double2 Bg[3];
 #pragma unroll
                 for (int x = 0; x < 3; x++) Bg[x] = __ldg(eB + 3 * c + x);
-#pragma unroll kBlkUnroll
                 for (int b = b0; b < b1; b++) {
                     const int4 m = bs.meta[b];
                     block_term(bs.M + 9 * b, Ag, Bg, bs.ph[phase_idx(d, qmx, m.y, m.z, m.w)], V);
@@ -151,73 +139,6 @@ __device__ __forceinline__ double2 contract_process(const FpDev &d, const BlkSme
     }
     return V;
 }
-#else
-// One block: t[y] = sum_x M[x][y] A[x];  W[y] += phase * t[y]                (12 complex MAC = 48 DFMA)
-// The three t chains are independent of every other block; only the 2-deep W update is carried from block to block.
-__device__ __forceinline__ void block_term(const double2 *M, const double2 *A, double2 ph, double2 *W) {
-#pragma unroll
-    for (int y = 0; y < 3; y++) {
-        double2 t = make_double2(0.0, 0.0);
-#pragma unroll
-        for (int x = 0; x < 3; x++) cfma(t, M[3 * x + y], A[x]);
-        cfma(W[y], t, ph);
-    }
-}
-
-// V = sum_c sum_y conj(e~_B(c,y)) W_c[y],  W_c[y] = sum_{b: atomB_b = c} phi(s2 qx, dR_b) sum_x Mhat_b[x][y] A(atomA_b, x).
-// Blocks are sorted by (atomB, atomA); bs.seg[c*nat + a] is the first block of the pair.  The B eigenvector is needed only
-// when a group closes, so it is fetched there (from L1: the caller prefetched it) instead of occupying registers.
-// NAT > 0: the A eigenvector lives in registers, block loop statically split by (atomB, atomA).
-// eA points at e~_A (s2=+) or conj(e~_A) (s2=-), eB at conj(e~_B); bs.ph holds phi (s2=+) or conj(phi) (s2=-): the
-// conjugations of step 6 are table choices made once per row, not arithmetic in the loop.
-template <int NAT>
-__device__ __forceinline__ double2 contract_process(const FpDev &d, const BlkSmem &bs, const double2 *__restrict__ eA,
-                                                    const double2 *__restrict__ eB, const double2 *A, const double2 *Bc,
-                                                    int3 qmx) {
-    double2 V = make_double2(0.0, 0.0);
-    if constexpr (NAT > 0) {
-#pragma unroll
-        for (int c = 0; c < NAT; c++) {
-            double2 W[3] = {make_double2(0.0, 0.0), make_double2(0.0, 0.0), make_double2(0.0, 0.0)};
-#pragma unroll
-            for (int a = 0; a < NAT; a++) {
-                const int b1 = bs.seg[c * NAT + a + 1];
-#pragma unroll kBlkUnroll
-                for (int b = bs.seg[c * NAT + a]; b < b1; b++) {
-                    const int4 m = bs.meta[b];
-                    block_term(bs.M + 9 * b, A + 3 * a, bs.ph[phase_idx(d, qmx, m.y, m.z, m.w)], W);
-                }
-            }
-#pragma unroll
-            for (int y = 0; y < 3; y++) cfma(V, W[y], FP_LATE_B ? __ldg(eB + 3 * c + y) : Bc[3 * c + y]);
-        }
-    } else {
-        const int nat = d.nat;
-        for (int c = 0; c < nat; c++) {
-            if (bs.seg[c * nat] == bs.seg[(c + 1) * nat]) continue;
-            double2 Bg[3];                                           // issued here, consumed after the group's blocks
-#pragma unroll
-            for (int y = 0; y < 3; y++) Bg[y] = __ldg(eB + 3 * c + y);
-            double2 W[3] = {make_double2(0.0, 0.0), make_double2(0.0, 0.0), make_double2(0.0, 0.0)};
-            for (int a = 0; a < nat; a++) {
-                const int b0 = bs.seg[c * nat + a], b1 = bs.seg[c * nat + a + 1];
-                if (b0 == b1) continue;
-                double2 Ag[3];
-#pragma unroll
-                for (int x = 0; x < 3; x++) Ag[x] = __ldg(eA + 3 * a + x);
-#pragma unroll kBlkUnroll
-                for (int b = b0; b < b1; b++) {
-                    const int4 m = bs.meta[b];
-                    block_term(bs.M + 9 * b, Ag, bs.ph[phase_idx(d, qmx, m.y, m.z, m.w)], W);
-                }
-            }
-#pragma unroll
-            for (int y = 0; y < 3; y++) cfma(V, W[y], Bg[y]);
-        }
-    }
-    return V;
-}
-#endif
 
 
 // Two processes per lane against one pass over the row's blocks: every Mhat_b read from shared memory feeds 2 x 13
@@ -255,9 +176,7 @@ __device__ __forceinline__ void contract_process2(const FpDev &d, const BlkSmem 
 // ---------------------------------------------------------------------------------------------------------------------
 // a2/a3 + a5/a6 + a7: fused enumerate -> shared-memory queue -> evaluate
 // ---------------------------------------------------------------------------------------------------------------------
-#ifndef FP_MINB
-#define FP_MINB 4                             // resident CTAs per SM the register allocation targets
-#endif
+constexpr int RATES_MINB = 4;                 // k_rates: 128 registers
 constexpr int RT = 128;                       // threads per row CTA
 constexpr int RW = RT / 32;                   // warps
 constexpr int PCAP = 32 + 32 * 36;            // pending queue: < 32 left over + one 6x6 sub-tile of 32 q-points
@@ -287,13 +206,7 @@ __device__ __forceinline__ void eval_process(const FpDev &d, const BlkSmem &bs, 
     double2 A[3 * (NAT > 0 ? NAT : 1)], Bc[3 * (NAT > 0 ? NAT : 1)];
     if constexpr (NAT > 0) {
         load_evec<3 * NAT>(eA, A);
-#if FP_BLK_FORM == 1 && FP_LATE_B
-#if !FP_EVAL_PF
-        prefetch_l1(eB); prefetch_l1(eB + 3 * NAT - 1);
-#endif
-#else
         load_evec<3 * NAT>(eB, Bc);
-#endif
     }
     // the decision, in the pinned arithmetic
     const double sig = sigma_pinned(d, a, b);
@@ -463,13 +376,14 @@ struct Steps {
 // process lists; the process lists of Algorithm 3, live and die in shared memory)
 // ---------------------------------------------------------------------------------------------------------------------
 template <int ORDER, int NAT, int TILE>
-__global__ void __launch_bounds__(RT, FP_MINB) k_rates(FpDev d, IfcDev f, RowArgs ra, const double2 *pre, double2 *partial,
-                                                 uint32_t *counts) {
+__global__ void __launch_bounds__(RT, RATES_MINB) k_rates(FpDev d, IfcDev f, RowArgs ra, const double2 *pre, double2 *partial,
+                                                 uint32_t *counts, bool only_flagged) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ double red[32];
     __shared__ unsigned redc[32];
     __shared__ int tailn[RW];
     const int64_t r = blockIdx.x;
+    if (only_flagged && counts[r] != 0xffffffffu) return;             // redo pass: only rows whose list slot filled up
     const Row row = make_row<ORDER>(d, ra, ra.row0 + r);
     if (!row.valid || row_is_empty(d, row)) {                         // item 8: zero modes are never a leg
         if (threadIdx.x == 0) { partial[r] = make_double2(0.0, 0.0); counts[r] = 0; }
@@ -644,14 +558,9 @@ __global__ void __launch_bounds__(RT, 8) k_enum(FpDev d, RowArgs ra, int64_t cap
 // Evaluator: |V|^2 of every listed process (level-2 contraction) and the row sums.  Every entry is an allowed process,
 // so the row count is the list length; the row factors of the weight (1/omega[omega'], occupation of lambda') multiply
 // the sums once.
-#ifndef FP_EVAL_PPL
-#define FP_EVAL_PPL 2                         // processes per lane of k_eval (NAT > 0): each Mhat read feeds two processes
-#endif
-#ifndef FP_EVAL_MINB
-#define FP_EVAL_MINB (FP_EVAL_PPL == 2 ? 3 : FP_MINB)
-#endif
+// k_eval: two processes per lane and 168 registers (NAT > 0: 3 CTAs per SM) or one and 128 (generic NAT == 0: 4 CTAs)
 template <int ORDER, int NAT>
-__global__ void __launch_bounds__(RT, FP_EVAL_MINB) k_eval(FpDev d, IfcDev f, RowArgs ra, const double2 *pre, int64_t capw,
+__global__ void __launch_bounds__(RT, (NAT > 0 ? 3 : 4)) k_eval(FpDev d, IfcDev f, RowArgs ra, const double2 *pre, int64_t capw,
                                                       const ListEnt *lists, const uint32_t *wcnt, double2 *partial,
                                                       uint32_t *counts) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -661,8 +570,8 @@ __global__ void __launch_bounds__(RT, FP_EVAL_MINB) k_eval(FpDev d, IfcDev f, Ro
     const bool ovf = (wc.x & wc.y & wc.z & wc.w) == 0xffffffffu || wc.x == 0xffffffffu || wc.y == 0xffffffffu ||
                      wc.z == 0xffffffffu || wc.w == 0xffffffffu;      // a slot of the row filled up: redone by k_rates
     const unsigned p1 = wc.x, p2 = p1 + wc.y, p3 = p2 + wc.z, total = ovf ? 0u : p3 + wc.w;
-    if (total == 0) {
-        if (threadIdx.x == 0) { partial[r] = make_double2(0.0, 0.0); counts[r] = 0; }
+    if (total == 0) {                                                 // (0xffffffff marks the row for the redo pass)
+        if (threadIdx.x == 0) { partial[r] = make_double2(0.0, 0.0); counts[r] = ovf ? 0xffffffffu : 0u; }
         return;
     }
     const Row row = make_row<ORDER>(d, ra, ra.row0 + r);
@@ -681,8 +590,7 @@ __global__ void __launch_bounds__(RT, FP_EVAL_MINB) k_eval(FpDev d, IfcDev f, Ro
         return e;
     };
     double sG = 0.0, sW = 0.0;
-#if FP_EVAL_PPL == 2
-    if constexpr (NAT > 0 && FP_BLK_FORM == 0) {
+    if constexpr (NAT > 0) {
         for (unsigned base = warp * 64; base < total; base += 2 * RT) {   // 64 processes per warp pass, two per lane
             const bool act0 = base + lane < total, act1 = base + 32 + lane < total;
             const ListEnt e0 = fetch(act0 ? base + lane : base), e1 = fetch(act1 ? base + 32 + lane : base);
@@ -700,7 +608,6 @@ __global__ void __launch_bounds__(RT, FP_EVAL_MINB) k_eval(FpDev d, IfcDev f, Ro
             if (act1) { sW += e1.w; sG = fma(e1.w, V1.x * V1.x + V1.y * V1.y, sG); }
         }
     } else
-#endif
     for (unsigned base = warp * 32; base < total; base += RT) {       // batch b of the row goes to warp b mod RW
         const bool act = base + lane < total;
         const ListEnt e = fetch(act ? base + lane : base);
@@ -757,20 +664,20 @@ static cudaError_t opt_in_smem(K kernel, size_t smem, size_t &granted) {   // op
 
 template <int ORDER, int NAT, int TILE>
 static cudaError_t launch_rates_t(const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const double2 *pre,
-                                  double2 *partial, uint32_t *counts, cudaStream_t st) {
+                                  double2 *partial, uint32_t *counts, bool only_flagged, cudaStream_t st) {
     const size_t smem = rates_smem_bytes(d, f);
     static size_t granted = 0;
     cudaError_t e = opt_in_smem(k_rates<ORDER, NAT, TILE>, smem, granted);
     if (e != cudaSuccess) return e;
-    k_rates<ORDER, NAT, TILE><<<(unsigned)nrows, RT, smem, st>>>(d, f, ra, pre, partial, counts);
+    k_rates<ORDER, NAT, TILE><<<(unsigned)nrows, RT, smem, st>>>(d, f, ra, pre, partial, counts, only_flagged);
     return cudaGetLastError();
 }
 
 cudaError_t launch_rates(int order, const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const double2 *pre,
-                         double2 *partial, uint32_t *counts, cudaStream_t st) {
+                         double2 *partial, uint32_t *counts, bool only_flagged, cudaStream_t st) {
     if (nrows <= 0) return cudaSuccess;
     const bool t6 = d.nb % 6 == 0;
-#define FP_ARGS d, f, ra, nrows, pre, partial, counts, st
+#define FP_ARGS d, f, ra, nrows, pre, partial, counts, only_flagged, st
     if (order == 3) {
         if (d.nat == 1) return launch_rates_t<3, 1, 3>(FP_ARGS);
         if (d.nat == 2) return launch_rates_t<3, 2, 6>(FP_ARGS);
