@@ -30,8 +30,8 @@ UNIT = "processes/s"
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12     # 148 SMs x 64 FP64 FMA/clk/SM x 2 flop x 1965 MHz
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed ncu --set full
 # captures (profiles/r1c_summary.md); keyed by (config, path).  None = not captured for that configuration.
-NCU_DRAM_BYTES_PER_LAUNCH = {(3, "split"): 569.7e6}   # k_eval<4,2>, a 10,922-row launch of config 3: 563.8 MB read (the
-#                                                        process list k_enum wrote) + 5.9 MB written
+NCU_DRAM_BYTES_PER_LAUNCH = {(3, "split"): 3.120e9}   # k_eval<4,2>, a 43,689-row launch of config 3: 3.105 GB read (the
+#                                                        process list k_enum wrote) + 15 MB written
 
 
 def workload(cfg: int):
@@ -277,14 +277,14 @@ def main():
     step_device()
     torch.cuda.synchronize()
     kern = {}
-    flops = procs = cands = pref = launches = rows = 0
+    flops = procs = cands = pref = launches = rows = overflows = 0
     for ctx in ctxs:
         p = ctx.profile_get()
         for k in ("precontract", "enum", "rates", "reduce"):
             kern.setdefault(k, [0.0, 0])
             kern[k][0] += getattr(p, "ms_" + k); kern[k][1] += getattr(p, "n_" + k)
         flops += p.rates_flops; procs += p.processes; cands += p.candidates; pref += p.prefiltered
-        launches += p.launches; rows += p.rows
+        launches += p.launches; rows += p.rows; overflows += p.list_overflows
         ctx.profile_enable(False)
     dom = max(kern, key=lambda k: kern[k][0])
     ms_c, n_c = kern["rates"]
@@ -297,7 +297,7 @@ def main():
     traffic = NCU_DRAM_BYTES_PER_LAUNCH.get((args.config, "split" if split else "fused"))
     roofline = {"bound": "alu", "kernel": kname, "achieved": achieved,
                 "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS, "traffic": traffic,
-                "traffic_source": "profiles/r1c_summary.md (ncu --set full, dram bytes read + written, one launch)"
+                "traffic_source": "profiles/r1d_summary.md (ncu --set full, dram bytes read + written, one launch)"
                                   if traffic is not None else None,
                 "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (MEASURED_PEAKS.json has no FP64 "
                                f"entry); DFMA probe on this GPU measured {probe:.2f} TFLOP/s",
@@ -308,7 +308,7 @@ def main():
                 "rows_per_step": rows, "candidates_per_step": cands, "prefiltered_per_step": pref,
                 "processes_per_step": procs,
                 "candidates_per_s_in_enumerator": cands / ((ms_en if split else ms_c) * 1e-3) if ms_c > 0 else 0.0,
-                "path": "split" if split else "fused"}
+                "path": "split" if split else "fused", "list_slot_overflows_per_step": overflows}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",

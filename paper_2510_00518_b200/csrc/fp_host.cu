@@ -11,6 +11,10 @@
 
 #include "fp_internal.cuh"
 
+#ifndef FP_SLOT_DIV
+#define FP_SLOT_DIV 4        // list slot = 1/FP_SLOT_DIV of the candidates a warp can meet
+#endif
+
 namespace {
 
 // ---- unit constants (SURVEY.md §8(c) "Constants"), derived from CODATA 2018 ------------------------------------------
@@ -429,7 +433,7 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
     // up is flagged by k_enum and its row is redone through the fused kernel (rows of the many-branch config 4, where
     // the +- channel admits 10 % and more of the candidates; never on the diamond configs)
     const int64_t capw_all = enum_slot_entries(d);
-    const int64_t capw = std::min(capw_all, std::max<int64_t>(((capw_all / 4) + 31) & ~(int64_t)31, 2048));
+    const int64_t capw = std::min(capw_all, std::max<int64_t>(((capw_all / FP_SLOT_DIV) + 31) & ~(int64_t)31, 2048));
     const size_t row_list_bytes = (size_t)enum_warps_per_row() * ((size_t)capw * sizeof(ListEnt) + sizeof(uint32_t));
     // FP_PATH_SPLIT runs the enumerator of chunk k+1 beside the evaluator of chunk k (two list buffers, two streams);
     // FP_PATH_SPLIT_SERIAL -- what FP_PATH_AUTO picks -- runs them back to back through one buffer of twice the rows.
