@@ -179,6 +179,8 @@ __device__ __forceinline__ void contract_process2(const FpDev &d, const BlkSmem 
 constexpr int RATES_MINB = 4;                 // k_rates: 128 registers
 constexpr int RT = 128;                       // threads per row CTA
 constexpr int RW = RT / 32;                   // warps
+constexpr int EVT = 128;                      // threads of a k_eval CTA (measured on B200, config 3: 32 -> 1363 ms, 64 -> 1232,
+                                              // 128 -> 1138, 256 -> 1425 per step: the row set-up wants several warps)
 constexpr int PCAP = 32 + 32 * 36;            // pending queue: < 32 left over + one 6x6 sub-tile of 32 q-points
 constexpr int QCAP = 64;                      // evaluation queue: < 32 left over + one stage-2 round
 
@@ -263,24 +265,24 @@ __device__ __forceinline__ unsigned char *setup_row_tables(const FpDev &d, const
     double2 *e1 = bs.ph + d.L;                                        // nb entries (level 1 of ORDER 4)
     bs.meta = reinterpret_cast<int4 *>(e1 + d.nb);
     bs.seg = reinterpret_cast<int *>(bs.meta + f.nblk);
-    for (int i = threadIdx.x; i < f.nblk; i += RT) bs.meta[i] = f.blk_meta[i];
-    for (int i = threadIdx.x; i <= d.nat * d.nat; i += RT) bs.seg[i] = f.seg[i];
+    for (int i = threadIdx.x; i < f.nblk; i += blockDim.x) bs.meta[i] = f.blk_meta[i];
+    for (int i = threadIdx.x; i <= d.nat * d.nat; i += blockDim.x) bs.seg[i] = f.seg[i];
     if (ORDER == 3) {
         const double2 *src = pre + (size_t)row.t * f.nblk * 9;
-        for (int i = threadIdx.x; i < f.nblk * 9; i += RT) bs.M[i] = src[i];
+        for (int i = threadIdx.x; i < f.nblk * 9; i += blockDim.x) bs.M[i] = src[i];
     } else {
         // level 1: Mhat_b[x][y] = sum_{c in b} phi(s1 q', Rj-Rl) sum_be T0[c][be][x][y] A'(j_c, be)
-        for (int i = threadIdx.x; i < d.L; i += RT) {
+        for (int i = threadIdx.x; i < d.L; i += blockDim.x) {
             double2 p = d.ph1d[i];
             if (row.s1 < 0) p.y = -p.y;
             bs.ph[i] = p;
         }
         const double2 *ev1 = (row.s1 > 0 ? d.evec : d.evecc) + (size_t)row.lam1 * d.nb;
-        for (int i = threadIdx.x; i < d.nb; i += RT) e1[i] = ev1[i];
+        for (int i = threadIdx.x; i < d.nb; i += blockDim.x) e1[i] = ev1[i];
         __syncthreads();
         const int3 qm1 = premul(d, unpack_qc(d.qc[row.lam1 / d.nb]));
         const double2 *T0 = pre + (size_t)row.t * f.n * 27;
-        for (int o = threadIdx.x; o < f.nblk * 9; o += RT) {
+        for (int o = threadIdx.x; o < f.nblk * 9; o += blockDim.x) {
             int b = o / 9, xy = o - 9 * b;
             double2 acc = make_double2(0.0, 0.0);
             for (int c = f.blk_start[b]; c < f.blk_start[b + 1]; c++) {
@@ -295,7 +297,7 @@ __device__ __forceinline__ unsigned char *setup_row_tables(const FpDev &d, const
         }
         __syncthreads();
     }
-    for (int i = threadIdx.x; i < d.L; i += RT) {                     // phases of the free legs: phi(s2 qx, dR)
+    for (int i = threadIdx.x; i < d.L; i += blockDim.x) {                     // phases of the free legs: phi(s2 qx, dR)
         double2 p = d.ph1d[i];
         if (row.s2 < 0) p.y = -p.y;
         bs.ph[i] = p;
@@ -511,14 +513,21 @@ __global__ void __launch_bounds__(RT, 8) k_enum(FpDev d, RowArgs ra, int64_t cap
                 wp -= n;
                 const bool in = lane < n;
                 const uint32_t c2 = pend[wp + (in ? lane : 0)];
-                uint2 e2;
-                const bool pass = prefilter2(d, row, basef, c2, e2) && in;
+                // stage 2 and the loads of stage 3 are issued together (one L2 round trip instead of two; a quarter of the
+                // FP64 records is fetched for candidates stage 2 then rejects)
+                const int qx = (int)(c2 >> 12), ja = (int)((c2 >> 6) & 63u), jb = (int)(c2 & 63u);
+                const int ql = q_index(d, q_add(d, row.qb, row.s2, unpack_qc(__ldg(d.qc + qx))));
+                const int p = qx * d.nb + ja, lamB = ql * d.nb + jb;
+                const uint2 e2 = make_uint2(((uint32_t)qx << 6) | (uint32_t)ja, ((uint32_t)ql << 6) | (uint32_t)jb);
+                const float4 Af = __ldg(d.recf + p), Bf = __ldg(d.recf + lamB);
+                const ModeRec a = load_rec(d.rec + p), b = load_rec(d.rec + lamB);
+                const double fa = __ldg(d.occ + p), fb = __ldg(d.occ + lamB);
+                const float dl = (row.s2 > 0 ? basef + Af.x : basef - Af.x) - Bf.x;
+                const float dx = Af.y - Bf.y, dy = Af.z - Bf.z, dz = Af.w - Bf.w;
+                const bool pass = in && dl * dl <= fmaf(d.pfK1, fmaf(dz, dz, fmaf(dy, dy, dx * dx)), d.pfC2);
                 bool ok = false;
                 double w = 0.0;
                 if (pass) {                                           // stage 3: the decision, in the pinned arithmetic
-                    const int p = (int)(e2.x >> 6) * d.nb + (int)(e2.x & 63u), lamB = (int)(e2.y >> 6) * d.nb + (int)(e2.y & 63u);
-                    const ModeRec a = load_rec(d.rec + p), b = load_rec(d.rec + lamB);
-                    const double fa = __ldg(d.occ + p), fb = __ldg(d.occ + lamB);
                     const double sig = sigma_pinned(d, a, b);
                     const double delta = __dsub_rn(row.s2 > 0 ? __dadd_rn(row.Obase, a.omega) : __dsub_rn(row.Obase, a.omega), b.omega);
                     ok = a.omega != 0.0 && b.omega != 0.0 && sig > 0.0 && fabs(delta) <= __dmul_rn(d.ncut, sig);
@@ -560,7 +569,7 @@ __global__ void __launch_bounds__(RT, 8) k_enum(FpDev d, RowArgs ra, int64_t cap
 // the sums once.
 // k_eval: two processes per lane and 168 registers (NAT > 0: 3 CTAs per SM) or one and 128 (generic NAT == 0: 4 CTAs)
 template <int ORDER, int NAT>
-__global__ void __launch_bounds__(RT, (NAT > 0 ? 3 : 4)) k_eval(FpDev d, IfcDev f, RowArgs ra, const double2 *pre, int64_t capw,
+__global__ void __launch_bounds__(EVT, (NAT > 0 ? 3 : 4) * (RT / EVT)) k_eval(FpDev d, IfcDev f, RowArgs ra, const double2 *pre, int64_t capw,
                                                       const ListEnt *lists, const uint32_t *wcnt, double2 *partial,
                                                       uint32_t *counts) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -591,7 +600,7 @@ __global__ void __launch_bounds__(RT, (NAT > 0 ? 3 : 4)) k_eval(FpDev d, IfcDev 
     };
     double sG = 0.0, sW = 0.0;
     if constexpr (NAT > 0) {
-        for (unsigned base = warp * 64; base < total; base += 2 * RT) {   // 64 processes per warp pass, two per lane
+        for (unsigned base = warp * 64; base < total; base += 2 * EVT) {   // 64 processes per warp pass, two per lane
             const bool act0 = base + lane < total, act1 = base + 32 + lane < total;
             const ListEnt e0 = fetch(act0 ? base + lane : base), e1 = fetch(act1 ? base + 32 + lane : base);
             const int qx0 = (int)(e0.x >> 6), qx1 = (int)(e1.x >> 6);
@@ -608,7 +617,7 @@ __global__ void __launch_bounds__(RT, (NAT > 0 ? 3 : 4)) k_eval(FpDev d, IfcDev 
             if (act1) { sW += e1.w; sG = fma(e1.w, V1.x * V1.x + V1.y * V1.y, sG); }
         }
     } else
-    for (unsigned base = warp * 32; base < total; base += RT) {       // batch b of the row goes to warp b mod RW
+    for (unsigned base = warp * 32; base < total; base += EVT) {      // batch b of the row goes to warp b mod (EVT/32)
         const bool act = base + lane < total;
         const ListEnt e = fetch(act ? base + lane : base);
         const int qx = (int)(e.x >> 6);
@@ -722,7 +731,7 @@ static cudaError_t launch_eval_t(const FpDev &d, const IfcDev &f, const RowArgs 
     static size_t granted = 0;
     cudaError_t e = opt_in_smem(k_eval<ORDER, NAT>, smem, granted);
     if (e != cudaSuccess) return e;
-    k_eval<ORDER, NAT><<<(unsigned)nrows, RT, smem, st>>>(d, f, ra, pre, capw, lists, wcnt, partial, counts);
+    k_eval<ORDER, NAT><<<(unsigned)nrows, EVT, smem, st>>>(d, f, ra, pre, capw, lists, wcnt, partial, counts);
     return cudaGetLastError();
 }
 
