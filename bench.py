@@ -253,7 +253,8 @@ def main():
     barrier()
     ms_total = e0.elapsed_time(e1)
     clocks = sampler.stop()
-    ms_step, procs_all = reduce_over_ranks(ms_total / args.steps, float(n4), dist if world > 1 else None)
+    counted = "4ph" if n4 > 0 else "3ph"                                  # configs 0 and 1 have no 4ph work: count 3ph processes
+    ms_step, procs_all = reduce_over_ranks(ms_total / args.steps, float(n4 if n4 > 0 else n3), dist if world > 1 else None)
     value = procs_all / (ms_step * 1e-3)
 
     # ---- end to end from host buffers ------------------------------------------------------------------------------------
@@ -314,7 +315,7 @@ def main():
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic",
             "config": {"workload": workload_name(args.config), "step": "fp_rates3 + fp_rates4 + fp_kappa_rta",
-                       "processes_4ph_per_step": n4, "processes_3ph_per_step": n3, "parallelism": f"replicas x{world}",
+                       "processes_4ph_per_step": n4, "processes_3ph_per_step": n3, "processes_counted_in_value": counted, "parallelism": f"replicas x{world}",
                        "l2": "flushed between steps (256 MB write)"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches * args.steps), "roofline": roofline}
     if rank == 0:
