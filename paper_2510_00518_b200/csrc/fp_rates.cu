@@ -173,6 +173,46 @@ __device__ __forceinline__ void contract_process2(const FpDev &d, const BlkSmem 
         }
 }
 
+// The same for any atom count: eigenvector components are fetched per atom group (A once per atomA, B once per
+// (atomA, atomB) pair with blocks), every Mhat_b read feeds both processes.
+__device__ __forceinline__ void contract_process2_generic(const FpDev &d, const BlkSmem &bs, const double2 *__restrict__ eA0,
+                                                          const double2 *__restrict__ eB0, int3 q0,
+                                                          const double2 *__restrict__ eA1, const double2 *__restrict__ eB1,
+                                                          int3 q1, double2 &V0, double2 &V1) {
+    V0 = make_double2(0.0, 0.0); V1 = make_double2(0.0, 0.0);
+    const int nat = d.nat;
+    for (int a = 0; a < nat; a++) {
+        if (bs.seg[a * nat] == bs.seg[(a + 1) * nat]) continue;
+        double2 A0[3], A1[3];
+#pragma unroll
+        for (int x = 0; x < 3; x++) { A0[x] = __ldg(eA0 + 3 * a + x); A1[x] = __ldg(eA1 + 3 * a + x); }
+        for (int c = 0; c < nat; c++) {
+            const int b0 = bs.seg[a * nat + c], b1 = bs.seg[a * nat + c + 1];
+            if (b0 == b1) continue;
+            double2 B0[3], B1[3];
+#pragma unroll
+            for (int y = 0; y < 3; y++) { B0[y] = __ldg(eB0 + 3 * c + y); B1[y] = __ldg(eB1 + 3 * c + y); }
+            for (int b = b0; b < b1; b++) {
+                const int4 m = bs.meta[b];
+                const double2 p0 = bs.ph[phase_idx(d, q0, m.y, m.z, m.w)], p1 = bs.ph[phase_idx(d, q1, m.y, m.z, m.w)];
+                const double2 *M = bs.M + 9 * b;
+                double2 u0 = make_double2(0.0, 0.0), u1 = make_double2(0.0, 0.0);
+#pragma unroll
+                for (int y = 0; y < 3; y++) {
+                    double2 t0 = make_double2(0.0, 0.0), t1 = make_double2(0.0, 0.0);
+#pragma unroll
+                    for (int x = 0; x < 3; x++) {
+                        const double2 mm = M[3 * x + y];
+                        cfma(t0, mm, A0[x]); cfma(t1, mm, A1[x]);
+                    }
+                    cfma(u0, t0, B0[y]); cfma(u1, t1, B1[y]);
+                }
+                cfma(V0, u0, p0); cfma(V1, u1, p1);
+            }
+        }
+    }
+}
+
 // ---------------------------------------------------------------------------------------------------------------------
 // a2/a3 + a5/a6 + a7: fused enumerate -> shared-memory queue -> evaluate
 // ---------------------------------------------------------------------------------------------------------------------
@@ -567,9 +607,9 @@ __global__ void __launch_bounds__(RT, 8) k_enum(FpDev d, RowArgs ra, int64_t cap
 // Evaluator: |V|^2 of every listed process (level-2 contraction) and the row sums.  Every entry is an allowed process,
 // so the row count is the list length; the row factors of the weight (1/omega[omega'], occupation of lambda') multiply
 // the sums once.
-// k_eval: two processes per lane and 168 registers (NAT > 0: 3 CTAs per SM) or one and 128 (generic NAT == 0: 4 CTAs)
+// k_eval: two processes per lane, 168 registers, 3 CTAs per SM
 template <int ORDER, int NAT>
-__global__ void __launch_bounds__(EVT, (NAT > 0 ? 3 : 4) * (RT / EVT)) k_eval(FpDev d, IfcDev f, RowArgs ra, const double2 *pre, int64_t capw,
+__global__ void __launch_bounds__(EVT, 3 * (RT / EVT)) k_eval(FpDev d, IfcDev f, RowArgs ra, const double2 *pre, int64_t capw,
                                                       const ListEnt *lists, const uint32_t *wcnt, double2 *partial,
                                                       uint32_t *counts) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -599,40 +639,25 @@ __global__ void __launch_bounds__(EVT, (NAT > 0 ? 3 : 4) * (RT / EVT)) k_eval(Fp
         return e;
     };
     double sG = 0.0, sW = 0.0;
-    if constexpr (NAT > 0) {
-        for (unsigned base = warp * 64; base < total; base += 2 * EVT) {   // 64 processes per warp pass, two per lane
-            const bool act0 = base + lane < total, act1 = base + 32 + lane < total;
-            const ListEnt e0 = fetch(act0 ? base + lane : base), e1 = fetch(act1 ? base + 32 + lane : base);
-            const int qx0 = (int)(e0.x >> 6), qx1 = (int)(e1.x >> 6);
-            const double2 *eA0 = (row.s2 > 0 ? d.evec : d.evecc) + ((size_t)qx0 * d.nb + (e0.x & 63u)) * d.nb;
-            const double2 *eA1 = (row.s2 > 0 ? d.evec : d.evecc) + ((size_t)qx1 * d.nb + (e1.x & 63u)) * d.nb;
-            const double2 *eB0 = d.evecc + ((size_t)(e0.y >> 6) * d.nb + (e0.y & 63u)) * d.nb;
-            const double2 *eB1 = d.evecc + ((size_t)(e1.y >> 6) * d.nb + (e1.y & 63u)) * d.nb;
-            const int3 xc0 = unpack_qc(__ldg(d.qc + qx0)), xc1 = unpack_qc(__ldg(d.qc + qx1));
+    for (unsigned base = warp * 64; base < total; base += 2 * EVT) {   // 64 processes per warp pass, two per lane
+        const bool act0 = base + lane < total, act1 = base + 32 + lane < total;
+        const ListEnt e0 = fetch(act0 ? base + lane : base), e1 = fetch(act1 ? base + 32 + lane : base);
+        const int qx0 = (int)(e0.x >> 6), qx1 = (int)(e1.x >> 6);
+        const double2 *eA0 = (row.s2 > 0 ? d.evec : d.evecc) + ((size_t)qx0 * d.nb + (e0.x & 63u)) * d.nb;
+        const double2 *eA1 = (row.s2 > 0 ? d.evec : d.evecc) + ((size_t)qx1 * d.nb + (e1.x & 63u)) * d.nb;
+        const double2 *eB0 = d.evecc + ((size_t)(e0.y >> 6) * d.nb + (e0.y & 63u)) * d.nb;
+        const double2 *eB1 = d.evecc + ((size_t)(e1.y >> 6) * d.nb + (e1.y & 63u)) * d.nb;
+        const int3 xc0 = unpack_qc(__ldg(d.qc + qx0)), xc1 = unpack_qc(__ldg(d.qc + qx1));
+        double2 V0, V1;
+        if constexpr (NAT > 0) {
             double2 A0[3 * (NAT > 0 ? NAT : 1)], B0[3 * (NAT > 0 ? NAT : 1)], A1[3 * (NAT > 0 ? NAT : 1)], B1[3 * (NAT > 0 ? NAT : 1)];
             load_evec<3 * NAT>(eA0, A0); load_evec<3 * NAT>(eB0, B0); load_evec<3 * NAT>(eA1, A1); load_evec<3 * NAT>(eB1, B1);
-            double2 V0, V1;
             contract_process2<NAT>(d, bs, A0, B0, premul(d, xc0), A1, B1, premul(d, xc1), V0, V1);
-            if (act0) { sW += e0.w; sG = fma(e0.w, V0.x * V0.x + V0.y * V0.y, sG); }
-            if (act1) { sW += e1.w; sG = fma(e1.w, V1.x * V1.x + V1.y * V1.y, sG); }
+        } else {
+            contract_process2_generic(d, bs, eA0, eB0, premul(d, xc0), eA1, eB1, premul(d, xc1), V0, V1);
         }
-    } else
-    for (unsigned base = warp * 32; base < total; base += EVT) {      // batch b of the row goes to warp b mod (EVT/32)
-        const bool act = base + lane < total;
-        const ListEnt e = fetch(act ? base + lane : base);
-        const int qx = (int)(e.x >> 6);
-        const int p = qx * d.nb + (int)(e.x & 63u), lamB = (int)(e.y >> 6) * d.nb + (int)(e.y & 63u);
-        const double2 *eA = (row.s2 > 0 ? d.evec : d.evecc) + (size_t)p * d.nb, *eB = d.evecc + (size_t)lamB * d.nb;
-        const int3 xc = unpack_qc(__ldg(d.qc + qx));
-        double2 A[3 * (NAT > 0 ? NAT : 1)], Bc[3 * (NAT > 0 ? NAT : 1)];
-        if constexpr (NAT > 0) {
-            load_evec<3 * NAT>(eA, A); load_evec<3 * NAT>(eB, Bc);
-        }
-        const double2 V = contract_process<NAT>(d, bs, eA, eB, A, Bc, premul(d, xc));
-        if (act) {
-            sW += e.w;
-            sG = fma(e.w, V.x * V.x + V.y * V.y, sG);
-        }
+        if (act0) { sW += e0.w; sG = fma(e0.w, V0.x * V0.x + V0.y * V0.y, sG); }
+        if (act1) { sW += e1.w; sG = fma(e1.w, V1.x * V1.x + V1.y * V1.y, sG); }
     }
     const double rowfac = rw.occ_row / rw.wrow;
     const double tG = block_sum<double>(sG, red);
