@@ -89,9 +89,11 @@ typedef struct {
     int64_t list_overflows; /* split path: (row, warp) list slots that filled up (their rows were redone fused)      */
 } fp_profile;
 
-/* Bytes of workspace fp_setup needs for its resident tables plus `scratch_bytes` of per-call scratch (per-target
- * pre-contracted tables and 20 bytes per row of partial sums; a larger scratch means fewer launches).  ifc3/ifc4 may
- * be NULL.  Returns 0 on invalid arguments.                                                                         */
+/* Bytes of workspace fp_setup needs for its resident tables plus `scratch_bytes` of per-call scratch: per-target
+ * pre-contracted tables, 20 bytes per row of partial sums and -- in half of it -- the process lists of the split path
+ * (4 x N x nb^2 bytes per row; a larger scratch means more rows per launch: 48 GB gives 43,689 rows at 16x16x16, nb = 6;
+ * below 256 rows of lists the fused path runs instead, see fp_set_path).  ifc3/ifc4 may be NULL.  Returns 0 on invalid
+ * arguments.                                                                                                          */
 size_t fp_workspace_bytes(const fp_crystal *crystal, const int32_t mesh[3], const fp_ifc *ifc3, const fp_ifc *ifc4,
                           size_t scratch_bytes);
 
