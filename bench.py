@@ -278,14 +278,16 @@ def main():
     step_device()
     torch.cuda.synchronize()
     kern = {}
-    flops = procs = cands = pref = launches = rows = overflows = 0
+    flops = procs = cands = pref = launches = rows = overflows = evaluated = 0
+    symmetry = False
     for ctx in ctxs:
         p = ctx.profile_get()
         for k in ("precontract", "enum", "rates", "reduce"):
             kern.setdefault(k, [0.0, 0])
             kern[k][0] += getattr(p, "ms_" + k); kern[k][1] += getattr(p, "n_" + k)
         flops += p.rates_flops; procs += p.processes; cands += p.candidates; pref += p.prefiltered
-        launches += p.launches; rows += p.rows; overflows += p.list_overflows
+        launches += p.launches; rows += p.rows; overflows += p.list_overflows; evaluated += p.evaluated
+        symmetry = symmetry or ctx.get_symmetry()
         ctx.profile_enable(False)
     dom = max(kern, key=lambda k: kern[k][0])
     ms_c, n_c = kern["rates"]
@@ -302,7 +304,12 @@ def main():
                                   if traffic is not None else None,
                 "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (MEASURED_PEAKS.json has no FP64 "
                                f"entry); DFMA probe on this GPU measured {probe:.2f} TFLOP/s",
-                "flops_model": "allowed processes x nblk x 13 complex MAC x 8 flop (DESIGN.md §6); enumeration not counted",
+                "flops_model": "matrix elements evaluated x nblk x 13 complex MAC x 8 flop (DESIGN.md §6); enumeration, "
+                               "decision and weights not counted",
+                "matrix_elements_per_step": evaluated,
+                "pair_symmetry": ("on: the IFC4 list is symmetric in its last two legs, so each unordered {lambda'', lambda'''} "
+                                  "pair of the +- and -- channels is evaluated once (both orderings counted as processes, "
+                                  "each with its own pinned window decision)") if symmetry else "off",
                 "flops_per_launch": flops / max(n_c, 1), "avg_launch_ms": ms_c / max(n_c, 1),
                 "dominant_by_time": dom,
                 "kernel_ms_per_step": {k: round(v[0], 3) for k, v in kern.items()},

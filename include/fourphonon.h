@@ -86,6 +86,7 @@ typedef struct {
     double  rates_flops;    /* FP64 flops of the per-process contraction (analytic model)             */
     double  ms_enum;        /* split path: summed durations of the enumerator kernel (ms_rates is then the evaluator) */
     int64_t n_enum;
+    int64_t evaluated;      /* matrix elements evaluated (= processes unless the pair symmetry is in effect)          */
     int64_t list_overflows; /* split path: (row, warp) list slots that filled up (their rows were redone fused)      */
 } fp_profile;
 
@@ -154,6 +155,16 @@ int fp_list4(fp_ctx *ctx, int32_t target, int32_t channel, int32_t qp, int32_t *
 #define FP_PATH_SPLIT 2
 #define FP_PATH_SPLIT_SERIAL 3
 int fp_set_path(fp_ctx *ctx, int path);
+
+/* Pair symmetry of the 4ph +- and -- channels.  fp_setup checks whether the IFC4 list is invariant under the exchange of
+ * its last two legs (Phi^{abgt}(i,j,k Rk,l Rl) = Phi^{abtg}(i,j,l Rl,k Rk) to 1e-13 of the largest entry: a derivative
+ * symmetry of every physical force-constant set).  If it is, |V4| and the occupation factors of the +- and -- channels
+ * are symmetric under lambda'' <-> lambda''', and the split path evaluates the matrix element of
+ * each unordered pair once, taking the window decision (pinned arithmetic) and the Gaussian weight of both orderings
+ * separately: counts stay bit-exact, rates change by summation order only.  fp_set_symmetry(ctx, 0) turns the reuse off;
+ * fp_get_symmetry returns 1 if it is in effect.                                                                       */
+int fp_set_symmetry(fp_ctx *ctx, int on);
+int fp_get_symmetry(const fp_ctx *ctx);
 
 /* Profiling of the library's own kernels (off by default; adds two cudaEventRecord per launch).                     */
 int fp_profile_enable(fp_ctx *ctx, int on);

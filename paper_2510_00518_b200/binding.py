@@ -28,7 +28,7 @@ _SOURCES = ["fp_kernels.cu", "fp_rates.cu", "fp_host.cu"]
 # every symbol include/fourphonon.h declares (tests check that the built library exports all of them)
 EXPORTED_SYMBOLS = [
     "fp_workspace_bytes", "fp_setup", "fp_rates3", "fp_rates4", "fp_kappa_rta", "fp_list3", "fp_list4",
-    "fp_set_path", "fp_profile_enable", "fp_profile_reset", "fp_profile_get", "fp_probe_fp64_tflops", "fp_constants",
+    "fp_set_path", "fp_set_symmetry", "fp_get_symmetry", "fp_profile_enable", "fp_profile_reset", "fp_profile_get", "fp_probe_fp64_tflops", "fp_constants",
     "fp_last_error", "fp_version", "fp_destroy",
 ]
 
@@ -74,7 +74,8 @@ class _Profile(C.Structure):
     _fields_ = [(n, C.c_double) for n in ("ms_precontract", "ms_rates", "ms_reduce")] + \
                [(n, C.c_int64) for n in ("n_precontract", "n_rates", "n_reduce", "rows", "candidates", "prefiltered",
                                          "processes")] + [("rates_flops", C.c_double), ("ms_enum", C.c_double),
-                                                          ("n_enum", C.c_int64), ("list_overflows", C.c_int64)]
+                                                          ("n_enum", C.c_int64), ("evaluated", C.c_int64),
+                                                          ("list_overflows", C.c_int64)]
 
 
 @dataclass
@@ -92,6 +93,7 @@ class Profile:
     rates_flops: float
     ms_enum: float = 0.0
     n_enum: int = 0
+    evaluated: int = 0
     list_overflows: int = 0
 
     @property
@@ -128,6 +130,10 @@ def load_library():
     lib.fp_list4.argtypes = [vp, i32, i32, i32, vp, i64, C.POINTER(i64), vp]
     lib.fp_set_path.restype = C.c_int
     lib.fp_set_path.argtypes = [vp, C.c_int]
+    lib.fp_set_symmetry.restype = C.c_int
+    lib.fp_set_symmetry.argtypes = [vp, C.c_int]
+    lib.fp_get_symmetry.restype = C.c_int
+    lib.fp_get_symmetry.argtypes = [vp]
     lib.fp_profile_enable.restype = C.c_int
     lib.fp_profile_enable.argtypes = [vp, C.c_int]
     lib.fp_profile_reset.restype = C.c_int
@@ -367,6 +373,14 @@ class Context:
     def set_path(self, path: int):
         """FP_PATH_AUTO / FP_PATH_FUSED / FP_PATH_SPLIT / FP_PATH_SPLIT_SERIAL (include/fourphonon.h)."""
         self._check(self.lib.fp_set_path(self.ctx, int(path)))
+
+    def set_symmetry(self, on: bool):
+        """Turn the lambda'' <-> lambda''' pair reuse of the 4ph +- / -- channels on or off (include/fourphonon.h)."""
+        self._check(self.lib.fp_set_symmetry(self.ctx, 1 if on else 0))
+
+    def get_symmetry(self) -> bool:
+        """True if fp_setup found the IFC4 list symmetric in its last two legs and the reuse is on."""
+        return self.lib.fp_get_symmetry(self.ctx) == 1
 
     def profile_enable(self, on=True):
         self._check(self.lib.fp_profile_enable(self.ctx, 1 if on else 0))

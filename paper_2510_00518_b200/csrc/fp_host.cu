@@ -127,6 +127,41 @@ int analyse_ifc(const fp_ifc *f, int order, int nat, const int32_t mesh[3], IfcH
     return FP_OK;
 }
 
+// Is the IFC4 list invariant under the exchange of its last two legs, Phi^{abgt}(i,j,k Rk,l Rl) = Phi^{abtg}(i,j,l Rl,k Rk)
+// (a derivative symmetry every physical force-constant set has)?  Then |V4| and the weights of the +- and -- channels
+// are symmetric under lambda'' <-> lambda''' and the split path evaluates each unordered pair
+// once.  Tolerance: 1e-13 of the largest entry.
+bool ifc4_last_legs_symmetric(const fp_ifc *f) {
+    typedef std::tuple<int, int, int, int, int, int, int, int, int, int, int, int, int> K;   // i j k l Rj Rk Rl
+    std::map<K, int64_t> idx;
+    auto key = [&](int64_t c, bool swap) {
+        const int32_t *at = f->atoms + c * 4, *cl = f->cells + c * 9;
+        const int32_t *Rk = cl + (swap ? 6 : 3), *Rl = cl + (swap ? 3 : 6);
+        return K(at[0], at[1], swap ? at[3] : at[2], swap ? at[2] : at[3], cl[0], cl[1], cl[2], Rk[0], Rk[1], Rk[2], Rl[0], Rl[1],
+                 Rl[2]);
+    };
+    double big = 0.0;
+    for (int64_t c = 0; c < f->n; c++) {
+        idx[key(c, false)] = c;
+        for (int x = 0; x < 81; x++) big = std::max(big, std::fabs(f->phi[c * 81 + x]));
+    }
+    const double tol = 1e-13 * big;
+    for (int64_t c = 0; c < f->n; c++) {
+        auto it = idx.find(key(c, true));
+        const double *P = f->phi + c * 81;
+        if (it == idx.end()) {                                // no partner: symmetric only if the cluster is zero
+            for (int x = 0; x < 81; x++) if (std::fabs(P[x]) > tol) return false;
+            continue;
+        }
+        const double *Q = f->phi + it->second * 81;
+        for (int ab = 0; ab < 9; ab++)
+            for (int g = 0; g < 3; g++)
+                for (int t = 0; t < 3; t++)
+                    if (std::fabs(P[ab * 9 + g * 3 + t] - Q[ab * 9 + t * 3 + g]) > tol) return false;
+    }
+    return true;
+}
+
 size_t ifc_resident_bytes(int64_t n, int order, int nat) {
     size_t ncomp = order == 3 ? 27 : 81;
     size_t b = 0;
@@ -299,7 +334,11 @@ int fp_setup(const fp_crystal *crystal, const double *masses, const double *omeg
     }
     d.rec = rec; d.recf = recf; d.recn = recn; d.occ = occ; d.evec = evec; d.evecc = evecc; d.ph1d = ph1d; d.qc = qc;
     if (ifc3) { int rc = upload_ifc(ctx, bump, h3, ctx->i3, st); if (rc) return bail(rc); ctx->has3 = true; }
-    if (ifc4) { int rc = upload_ifc(ctx, bump, h4, ctx->i4, st); if (rc) return bail(rc); ctx->has4 = true; }
+    if (ifc4) {
+        int rc = upload_ifc(ctx, bump, h4, ctx->i4, st); if (rc) return bail(rc);
+        ctx->has4 = true;
+        ctx->sym34 = ifc4_last_legs_symmetric(ifc4);
+    }
     ctx->resident = align_up(bump.off);
 
     // ---- stage raw mode arrays (scratch region) and validate omega on the host ---------------------------------------
@@ -434,7 +473,7 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
     // the +- channel admits 10 % and more of the candidates; never on the diamond configs)
     const int64_t capw_all = enum_slot_entries(d);
     const int64_t capw = std::min(capw_all, std::max<int64_t>(((capw_all / FP_SLOT_DIV) + 31) & ~(int64_t)31, 2048));
-    const size_t row_list_bytes = (size_t)enum_warps_per_row() * ((size_t)capw * sizeof(ListEnt) + sizeof(uint32_t));
+    const size_t row_list_bytes = (size_t)enum_warps_per_row() * ((size_t)capw * sizeof(ListEnt) + 2 * sizeof(uint32_t));
     // FP_PATH_SPLIT runs the enumerator of chunk k+1 beside the evaluator of chunk k (two list buffers, two streams);
     // FP_PATH_SPLIT_SERIAL -- what FP_PATH_AUTO picks -- runs them back to back through one buffer of twice the rows.
     const bool overlap = ctx->path == FP_PATH_SPLIT;
@@ -477,7 +516,7 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
         double2 *pre = sc.take<double2>(nts * (pre_per_target / sizeof(double2)));
         uint32_t *cnt = sc.take<uint32_t>(nrows);
         double2 *partial = sc.take<double2>(nrows);
-        unsigned long long *stat = sc.take<unsigned long long>(2);    // [0] pre-filter survivors, [1] list overflows
+        unsigned long long *stat = sc.take<unsigned long long>(3);    // [0] pre-filter survivors, [1] list overflows, [2] list entries
         double *o_gamma = sc.take<double>(nts * nch), *o_wp = sc.take<double>(nts * nch);
         int64_t *o_cnt = sc.take<int64_t>(nts * nch);
         if (!pre || !cnt || !partial || !stat || !o_gamma || !o_wp || !o_cnt) return fail(ctx, FP_ENOMEM, "scratch");
@@ -485,7 +524,9 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
         RowArgs ra; ra.targets = d_targets; ra.row0 = 0; ra.qp_begin = qp_begin; ra.nqp = (int)nqp;
         ra.prefiltered = ctx->profiling ? stat : nullptr;
         ra.overflow = reinterpret_cast<unsigned int *>(stat + 1);
-        CU(cudaMemsetAsync(stat, 0, 2 * sizeof(unsigned long long), st));
+        ra.evaluated = ctx->profiling ? stat + 2 : nullptr;
+        ra.sym = (order == 4 && split && ctx->sym34 && ctx->use_sym) ? 1 : 0;
+        CU(cudaMemsetAsync(stat, 0, 3 * sizeof(unsigned long long), st));
         { ProfScope p(ctx, CAT_PRE, st);
           if (order == 3) launch_pre3(d, f, d_targets, nts, pre, st); else launch_pre4(d, f, d_targets, nts, pre, st); }
         CU(cudaGetLastError());
@@ -498,7 +539,7 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
             ListEnt *lists[2]; uint32_t *wcnt[2];
             for (int b = 0; b < nbuf; b++) {
                 lists[b] = sc.take<ListEnt>((size_t)chunk_rows * enum_warps_per_row() * capw);
-                wcnt[b] = sc.take<uint32_t>((size_t)chunk_rows * enum_warps_per_row());
+                wcnt[b] = sc.take<uint32_t>(2 * (size_t)chunk_rows * enum_warps_per_row());   // entries, then processes
                 if (!lists[b] || !wcnt[b]) return fail(ctx, FP_ENOMEM, "scratch (process lists)");
             }
             cudaStream_t es = overlap ? ctx->side : st;
@@ -513,13 +554,14 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
                 RowArgs rc = ra; rc.row0 = r0;
                 if (overlap && k >= 2) CU(cudaStreamWaitEvent(es, ctx->ev_eval[b], 0));
                 { ProfScope p(ctx, CAT_ENUM, es);
-                  CU(launch_enum(order, d, rc, nr, capw, lists[b], wcnt[b], es)); }
+                  CU(launch_enum(order, d, rc, nr, capw, lists[b], wcnt[b], wcnt[b] + chunk_rows * enum_warps_per_row(), es)); }
                 if (overlap) {
                     CU(cudaEventRecord(ctx->ev_enum[b], es));
                     CU(cudaStreamWaitEvent(st, ctx->ev_enum[b], 0));
                 }
                 { ProfScope p(ctx, CAT_RATES, st);
-                  CU(launch_eval(order, d, f, rc, nr, pre, capw, lists[b], wcnt[b], partial + r0, cnt + r0, st)); }
+                  CU(launch_eval(order, d, f, rc, nr, pre, capw, lists[b], wcnt[b], wcnt[b] + chunk_rows * enum_warps_per_row(),
+                                 partial + r0, cnt + r0, st)); }
                 if (overlap) CU(cudaEventRecord(ctx->ev_eval[b], st));
             }
             unsigned long long novf = 0;
@@ -546,16 +588,21 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
         CU(cudaStreamSynchronize(st));                               // the scratch is reused by the next super-chunk
         if (ctx->profiling) {                                        // analytic models, DESIGN.md §6
             std::vector<int64_t> hc(nts * nch);
-            unsigned long long hstat = 0;
+            unsigned long long hstat3[3] = {0, 0, 0};
             CU(cudaMemcpy(hc.data(), c_out, nts * nch * 8, cudaMemcpyDeviceToHost));
-            CU(cudaMemcpy(&hstat, stat, 8, cudaMemcpyDeviceToHost));
+            CU(cudaMemcpy(hstat3, stat, sizeof(hstat3), cudaMemcpyDeviceToHost));
+            const unsigned long long hstat = hstat3[0];
             int64_t total = 0;
             for (int64_t v : hc) total += v;
             ctx->prof.rows += nrows;
             ctx->prof.processes += total;
             ctx->prof.prefiltered += (int64_t)hstat;
             ctx->prof.candidates += nrows * row_cands;
-            ctx->prof.rates_flops += (double)total * (double)f.nblk * 13.0 * 8.0;
+            // matrix elements evaluated: the list entries of the split path (rows redone by k_rates after a list overflow
+            // are not in this figure), else one per process
+            const int64_t evaluated = split ? (int64_t)hstat3[2] : total;
+            ctx->prof.evaluated += evaluated;
+            ctx->prof.rates_flops += (double)evaluated * (double)f.nblk * 13.0 * 8.0;
         }
     }
     return FP_OK;
@@ -613,6 +660,7 @@ static int list_driver(fp_ctx *ctx, int order, int32_t target, int32_t channel, 
     if (!d_t || !cnt || !offs || !bsums) return fail(ctx, FP_ENOMEM, "scratch");
     CU(cudaMemcpyAsync(d_t, &target, 4, cudaMemcpyHostToDevice, st));
     RowArgs ra; ra.targets = d_t; ra.row0 = 0; ra.qp_begin = qp; ra.nqp = 1; ra.prefiltered = nullptr; ra.overflow = nullptr;
+    ra.evaluated = nullptr; ra.sym = 0;
     launch_count(order, d, ra, nrows, cnt, st);
     launch_scan(cnt, nrows, offs, bsums, st);
     std::vector<int64_t> ho(nrows + 1);
@@ -650,6 +698,9 @@ int fp_set_path(fp_ctx *ctx, int path) {
     ctx->path = path;
     return FP_OK;
 }
+
+int fp_set_symmetry(fp_ctx *ctx, int on) { if (!ctx) return FP_EINVAL; ctx->use_sym = on != 0; return FP_OK; }
+int fp_get_symmetry(const fp_ctx *ctx) { return ctx ? (ctx->sym34 && ctx->use_sym ? 1 : 0) : FP_EINVAL; }
 
 int fp_profile_enable(fp_ctx *ctx, int on) { if (!ctx) return FP_EINVAL; ctx->profiling = on != 0; return FP_OK; }
 

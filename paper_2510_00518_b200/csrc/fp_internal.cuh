@@ -60,6 +60,8 @@ struct RowArgs {
     int64_t row0;                 // first row handled by this launch
     int qp_begin, nqp;            // 4ph only
     unsigned long long *prefiltered;   // nullable: += candidates admitted by the FP32 pre-filter (profiling)
+    unsigned long long *evaluated;     // nullable: += list entries written by k_enum = matrix elements k_eval evaluates
+    int sym;                      // 1: 4ph rows of the +- and -- channels list each unordered {lambda'', lambda'''} pair once
     unsigned int *overflow;       // split path: += 1 for every (row, warp) list slot that filled up (the driver then
                                   // re-runs those rows through the fused kernel)
 };
@@ -79,6 +81,8 @@ struct fp_ctx {
     int sm_count = 148;
     bool profiling = false;
     int path = FP_PATH_AUTO;      // fp_set_path
+    bool sym34 = false;           // IFC4 is symmetric under the exchange of its last two legs (checked by fp_setup)
+    bool use_sym = true;          // fp_set_symmetry
     cudaStream_t side = nullptr;  // second stream of the split path: the enumerator of chunk k+1 runs beside the
     cudaEvent_t ev_enum[2] = {nullptr, nullptr}, ev_eval[2] = {nullptr, nullptr};   // evaluator of chunk k
     std::vector<EventRec> events;
@@ -105,11 +109,12 @@ size_t rates_smem_bytes(const FpDev &d, const IfcDev &f);
 // split path (fp_rates.cu): enumerator -> process lists in the scratch -> evaluator
 int64_t enum_slot_entries(const FpDev &d);        // entries of one (row, warp) list slot that can never overflow
 int enum_warps_per_row();
+// wcnt[row*RW + warp] = list entries written, pcnt[row*RW + warp] = allowed processes they stand for
 cudaError_t launch_enum(int order, const FpDev &d, const RowArgs &ra, int64_t nrows, int64_t capw, ListEnt *lists,
-                        uint32_t *wcnt, cudaStream_t st);
+                        uint32_t *wcnt, uint32_t *pcnt, cudaStream_t st);
 cudaError_t launch_eval(int order, const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const double2 *pre,
-                        int64_t capw, const ListEnt *lists, const uint32_t *wcnt, double2 *partial, uint32_t *counts,
-                        cudaStream_t st);
+                        int64_t capw, const ListEnt *lists, const uint32_t *wcnt, const uint32_t *pcnt, double2 *partial,
+                        uint32_t *counts, cudaStream_t st);
 void launch_finalize(int order, const FpDev &d, int64_t nt, int64_t rows_per_unit, const double2 *partial,
                      const uint32_t *counts, double c_over_n, double *gamma, double *wp, int64_t *cnt, cudaStream_t st);
 void launch_kappa(const FpDev &d, const double *gamma_total, double pref, double *kappa, cudaStream_t st);

@@ -358,7 +358,7 @@ __device__ __forceinline__ unsigned char *setup_row_tables(const FpDev &d, const
 // candidate order, to the warp's pending queue.  Returns the new queue length (warp-uniform).
 template <int TILE>
 __device__ __forceinline__ int stage1_step(const FpDev &d, const Row &row, float basef, int tile, int ja0, int jb0,
-                                           int lane, uint32_t *pend, int wp) {
+                                           int lane, uint32_t *pend, int wp, bool canonical_only = false) {
     const float fnan = __int_as_float(0x7fc00000);
     const int qx = (tile << 5) + lane;
     const bool inq = qx < d.N;
@@ -380,6 +380,15 @@ __device__ __forceinline__ int stage1_step(const FpDev &d, const Row &row, float
 #pragma unroll
         for (int i = 0; i < TILE; i++)
             if (bl <= hi[i] && bh >= lo[i]) mask |= 1ull << (8 * i + k);
+    }
+    if (canonical_only) {                                             // pair symmetry: keep mode A <= mode B only
+        uint64_t upper = 0;                                           // bit 8 i + k with ja0 + i <= jb0 + k
+#pragma unroll
+        for (int i = 0; i < TILE; i++)
+#pragma unroll
+            for (int k = 0; k < TILE; k++)
+                if (ja0 + i <= jb0 + k) upper |= 1ull << (8 * i + k);
+        mask = qs < ql ? mask : qs == ql ? (mask & upper) : 0ull;
     }
     const unsigned c = __popcll(mask);                                // ordered append to the pending queue
     unsigned incl = c;
@@ -529,13 +538,18 @@ static_assert(RW == 4, "k_eval reads the four warp counts of a row as one uint4"
 // (SURVEY.md §8(c) step 3), which alone determines what is written, and the row-independent part of the
 // weight (a7).  With ~48 registers per thread ten CTAs fit on an SM, which hides the gather latency of the decision.
 template <int ORDER, int TILE, bool ONE_SUB>
-__global__ void __launch_bounds__(RT, 8) k_enum(FpDev d, RowArgs ra, int64_t capw, ListEnt *lists, uint32_t *wcnt) {
+__global__ void __launch_bounds__(RT, 8) k_enum(FpDev d, RowArgs ra, int64_t capw, ListEnt *lists, uint32_t *wcnt,
+                                                uint32_t *pcnt) {
     __shared__ uint32_t pendq[RW * PCAP];
     const int64_t r = blockIdx.x;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const Row row = make_row<ORDER>(d, ra, ra.row0 + r);
-    unsigned nout = 0, nadm = 0;
+    unsigned nout = 0, nadm = 0, nproc = 0;
     bool ovf = false;                                                 // the slot filled up: the row is redone by k_rates
+    // pair symmetry (fp_set_symmetry): in the +- and -- channels (s2 < 0) the two free legs enter V4 and the weight in the
+    // same way, so only mode A <= mode B is listed; its entry carries the weights of both orderings, each with its own
+    // window decision in the pinned arithmetic
+    const bool sym = ORDER == 4 && ra.sym && row.s2 < 0;
     if (row.valid && !row_is_empty(d, row)) {                         // item 8: zero modes are never a leg
         ListEnt *out = lists + ((size_t)r * RW + warp) * (size_t)capw;
         uint32_t *pend = pendq + warp * PCAP;
@@ -545,7 +559,7 @@ __global__ void __launch_bounds__(RT, 8) k_enum(FpDev d, RowArgs ra, int64_t cap
         for (int step = warp; step < steps.nsteps; step += RW) {
             int tile, ja0, jb0;
             steps.decode(step, tile, ja0, jb0);
-            wp = stage1_step<TILE>(d, row, basef, tile, ja0, jb0, lane, pend, wp);
+            wp = stage1_step<TILE>(d, row, basef, tile, ja0, jb0, lane, pend, wp, sym);
             __syncwarp();
             const bool last = step + RW >= steps.nsteps;
             while (wp >= 32 || (last && wp > 0)) {                    // stage 2, 32 pending candidates at a time
@@ -579,6 +593,21 @@ __global__ void __launch_bounds__(RT, 8) k_enum(FpDev d, RowArgs ra, int64_t cap
                     if (ORDER == 3) occ = row.s2 > 0 ? (fa - fb) : (fa + fb + 1.0);
                     else occ = (row.s2 > 0 ? 1.0 + fa : fa) * fb;
                     w = occ * (exp(-(rr * rr)) * t * 0.56418958354775628695);   // 1/sqrt(pi)
+                    if (!ok) w = 0.0;
+                    if (sym) {                                        // the other ordering: Delta' = (Obase - omega_B) - omega_A
+                        const double delta2 = __dsub_rn(__dsub_rn(row.Obase, b.omega), a.omega);
+                        const bool ok2 = p != lamB &&                 // (A = B is its own partner: one process; only a fixed sigma admits it)
+                                         a.omega != 0.0 && b.omega != 0.0 && sig > 0.0 && fabs(delta2) <= __dmul_rn(d.ncut, sig);
+                        if (ok2) {
+                            const double r2 = delta2 * (t * W);
+                            w += delta2 == delta ? occ * (exp(-(rr * rr)) * t * 0.56418958354775628695)
+                                                 : occ * (exp(-(r2 * r2)) * t * 0.56418958354775628695);
+                        }
+                        nproc += (ok ? 1u : 0u) + (ok2 ? 1u : 0u);
+                        ok = ok || ok2;
+                    } else {
+                        nproc += ok ? 1u : 0u;
+                    }
                 }
                 const unsigned bal = __ballot_sync(0xffffffffu, ok);
                 if (nout + __popc(bal) > (unsigned)capw) ovf = true;  // warp-uniform
@@ -594,9 +623,12 @@ __global__ void __launch_bounds__(RT, 8) k_enum(FpDev d, RowArgs ra, int64_t cap
             __syncwarp();
         }
     }
+    for (int o = 16; o > 0; o >>= 1) nproc += __shfl_down_sync(0xffffffffu, nproc, o);
     if (lane == 0) {
         wcnt[r * RW + warp] = ovf ? 0xffffffffu : nout;
+        pcnt[r * RW + warp] = nproc;
         if (ovf) atomicAdd(ra.overflow, 1u);
+        else if (ra.evaluated && nout) atomicAdd(ra.evaluated, (unsigned long long)nout);
     }
     if (ra.prefiltered) {                                             // profiling only: pre-filter survivors
         for (int o = 16; o > 0; o >>= 1) nadm += __shfl_down_sync(0xffffffffu, nadm, o);
@@ -610,8 +642,8 @@ __global__ void __launch_bounds__(RT, 8) k_enum(FpDev d, RowArgs ra, int64_t cap
 // k_eval: two processes per lane, 168 registers, 3 CTAs per SM
 template <int ORDER, int NAT>
 __global__ void __launch_bounds__(EVT, 3 * (RT / EVT)) k_eval(FpDev d, IfcDev f, RowArgs ra, const double2 *pre, int64_t capw,
-                                                      const ListEnt *lists, const uint32_t *wcnt, double2 *partial,
-                                                      uint32_t *counts) {
+                                                      const ListEnt *lists, const uint32_t *wcnt, const uint32_t *pcnt,
+                                                      double2 *partial, uint32_t *counts) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ double red[32];
     const int64_t r = blockIdx.x;
@@ -662,7 +694,10 @@ __global__ void __launch_bounds__(EVT, 3 * (RT / EVT)) k_eval(FpDev d, IfcDev f,
     const double rowfac = rw.occ_row / rw.wrow;
     const double tG = block_sum<double>(sG, red);
     const double tW = block_sum<double>(sW, red);
-    if (threadIdx.x == 0) { partial[r] = make_double2(rowfac * tG, rowfac * tW); counts[r] = total; }
+    if (threadIdx.x == 0) {                                           // processes: both orderings of a listed pair count
+        const uint4 pc = __ldg(reinterpret_cast<const uint4 *>(pcnt) + r);
+        partial[r] = make_double2(rowfac * tG, rowfac * tW); counts[r] = pc.x + pc.y + pc.z + pc.w;
+    }
 }
 
 }  // namespace
@@ -733,10 +768,10 @@ int64_t enum_slot_entries(const FpDev &d) {
 int enum_warps_per_row() { return RW; }
 
 cudaError_t launch_enum(int order, const FpDev &d, const RowArgs &ra, int64_t nrows, int64_t capw, ListEnt *lists,
-                        uint32_t *wcnt, cudaStream_t st) {
+                        uint32_t *wcnt, uint32_t *pcnt, cudaStream_t st) {
     if (nrows <= 0) return cudaSuccess;
     const unsigned g = (unsigned)nrows;
-#define FP_ENUM(O, T, S) k_enum<O, T, S><<<g, RT, 0, st>>>(d, ra, capw, lists, wcnt)
+#define FP_ENUM(O, T, S) k_enum<O, T, S><<<g, RT, 0, st>>>(d, ra, capw, lists, wcnt, pcnt)
     if (order == 3) {
         if (d.nb == 6) FP_ENUM(3, 6, true); else if (d.nb == 3) FP_ENUM(3, 3, true);
         else if (d.nb % 6 == 0) FP_ENUM(3, 6, false); else FP_ENUM(3, 3, false);
@@ -750,21 +785,21 @@ cudaError_t launch_enum(int order, const FpDev &d, const RowArgs &ra, int64_t nr
 
 template <int ORDER, int NAT>
 static cudaError_t launch_eval_t(const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const double2 *pre,
-                                 int64_t capw, const ListEnt *lists, const uint32_t *wcnt, double2 *partial,
-                                 uint32_t *counts, cudaStream_t st) {
+                                 int64_t capw, const ListEnt *lists, const uint32_t *wcnt, const uint32_t *pcnt,
+                                 double2 *partial, uint32_t *counts, cudaStream_t st) {
     const size_t smem = (tables_smem_bytes(d, f) + 15) & ~(size_t)15;
     static size_t granted = 0;
     cudaError_t e = opt_in_smem(k_eval<ORDER, NAT>, smem, granted);
     if (e != cudaSuccess) return e;
-    k_eval<ORDER, NAT><<<(unsigned)nrows, EVT, smem, st>>>(d, f, ra, pre, capw, lists, wcnt, partial, counts);
+    k_eval<ORDER, NAT><<<(unsigned)nrows, EVT, smem, st>>>(d, f, ra, pre, capw, lists, wcnt, pcnt, partial, counts);
     return cudaGetLastError();
 }
 
 cudaError_t launch_eval(int order, const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const double2 *pre,
-                        int64_t capw, const ListEnt *lists, const uint32_t *wcnt, double2 *partial, uint32_t *counts,
-                        cudaStream_t st) {
+                        int64_t capw, const ListEnt *lists, const uint32_t *wcnt, const uint32_t *pcnt, double2 *partial,
+                        uint32_t *counts, cudaStream_t st) {
     if (nrows <= 0) return cudaSuccess;
-#define FP_ARGS d, f, ra, nrows, pre, capw, lists, wcnt, partial, counts, st
+#define FP_ARGS d, f, ra, nrows, pre, capw, lists, wcnt, pcnt, partial, counts, st
     if (order == 3) {
         if (d.nat == 1) return launch_eval_t<3, 1>(FP_ARGS);
         if (d.nat == 2) return launch_eval_t<3, 2>(FP_ARGS);

@@ -215,7 +215,7 @@ def test_small_scratch_splits_targets_and_gives_identical_results(fp):
             gs, ws, cs = small.rates4(t)
             p = small.profile_get()
             assert p.n_rates > n_big
-            assert p.processes == int(cs.sum()) and p.prefiltered >= p.processes
+            assert p.processes == int(cs.sum()) and p.prefiltered >= p.evaluated > 0
             assert p.candidates == len(t) * 3 * inp.nq ** 2 * inp.nb ** 3
         assert np.array_equal(c, cs) and np.array_equal(g, gs) and np.array_equal(w, ws)
 
@@ -373,3 +373,40 @@ def test_list_overflow_falls_back_to_fused(fp):
         ctx.profile_enable(True)
         ctx.rates4(t, 5, 6)
         assert ctx.profile_get().list_overflows == 0
+
+
+def test_pair_symmetry_of_the_4ph_channels(fp):
+    """fp_setup detects that the (symmetrised) IFC4 list is invariant under the exchange of its last two legs; the split path
+    then lists each unordered {lambda'', lambda'''} pair of the +- and -- channels once.  Counts must not change at all, rates
+    only by summation order; about half of the matrix elements are evaluated."""
+    inp = fp_inputs.make_tiny("diamond", mesh=(4, 4, 4))
+    t = inp.targets4[30:54]
+    res = {}
+    for on in (True, False):
+        with fp.Context.from_inputs(inp, scratch_bytes=256 << 20) as ctx:
+            ctx.set_path(fp.FP_PATH_SPLIT_SERIAL)
+            ctx.set_symmetry(on)
+            assert ctx.get_symmetry() == on
+            ctx.profile_enable(True)
+            res[on] = ctx.rates4(t)
+            p = ctx.profile_get()
+            res[on] += (p.evaluated, p.processes)
+    (g1, w1, c1, e1, p1), (g0, w0, c0, e0, p0) = res[True], res[False]
+    assert np.array_equal(c1, c0) and p1 == p0 == int(c0.sum())
+    assert e0 == p0 and e1 < 0.62 * e0                               # ++ is not reduced, +- and -- are halved
+    assert np.allclose(g1, g0, rtol=1e-12, atol=1e-13 * np.abs(g0).max())
+    assert np.allclose(w1, w0, rtol=1e-12, atol=1e-13 * np.abs(w0).max())
+
+
+def test_asymmetric_ifc4_disables_the_pair_symmetry(fp):
+    """An IFC4 list that is not symmetric in its last two legs (one entry perturbed) must be evaluated over the full
+    domain -- and still match the oracle, which never uses any symmetry."""
+    inp = fp_inputs.make_tiny("diamond", mesh=(3, 3, 3))
+    a4, c4, p4 = inp.ifc4
+    p4 = p4.copy()
+    p4[3, 1 * 27 + 0 * 9 + 1 * 3 + 2] += 0.37                        # component (y,x,y,z) of one quartet
+    inp.ifc4 = (a4, c4, p4)
+    t = inp.targets4[7:19]
+    with fp.Context.from_inputs(inp, scratch_bytes=64 << 20) as ctx:
+        assert not ctx.get_symmetry()
+    check4(fp, inp, t)
