@@ -30,8 +30,8 @@ UNIT = "processes/s"
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12     # 148 SMs x 64 FP64 FMA/clk/SM x 2 flop x 1965 MHz
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed ncu --set full
 # captures (profiles/r1c_summary.md); keyed by (config, path).  None = not captured for that configuration.
-NCU_DRAM_BYTES_PER_LAUNCH = {(3, "split"): 3.120e9}   # k_eval<4,2>, a 43,689-row launch of config 3: 3.105 GB read (the
-#                                                        process list k_enum wrote) + 15 MB written
+NCU_DRAM_BYTES_PER_LAUNCH = {(3, "split"): 1.562e9}   # k_eval<4,2>, a 43,688-row launch of config 3: 1.556 GB read (the
+#                                                        process list k_enum wrote) + 6 MB written
 
 
 def workload(cfg: int):
@@ -300,7 +300,7 @@ def main():
     traffic = NCU_DRAM_BYTES_PER_LAUNCH.get((args.config, "split" if split else "fused"))
     roofline = {"bound": "alu", "kernel": kname, "achieved": achieved,
                 "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS, "traffic": traffic,
-                "traffic_source": "profiles/r1d_summary.md (ncu --set full, dram bytes read + written, one launch)"
+                "traffic_source": "profiles/r1f_summary.md (ncu --set full, dram bytes read + written, one launch)"
                                   if traffic is not None else None,
                 "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (MEASURED_PEAKS.json has no FP64 "
                                f"entry); DFMA probe on this GPU measured {probe:.2f} TFLOP/s",
