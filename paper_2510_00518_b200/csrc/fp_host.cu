@@ -142,7 +142,7 @@ bool ifc4_last_legs_symmetric(const fp_ifc *f) {
     };
     double big = 0.0;
     for (int64_t c = 0; c < f->n; c++) {
-        idx[key(c, false)] = c;
+        if (!idx.emplace(key(c, false), c).second) return false;   // duplicate cluster: do not reason about sums, stay safe
         for (int x = 0; x < 81; x++) big = std::max(big, std::fabs(f->phi[c * 81 + x]));
     }
     const double tol = 1e-13 * big;

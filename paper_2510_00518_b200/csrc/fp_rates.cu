@@ -364,6 +364,9 @@ __device__ __forceinline__ int stage1_step(const FpDev &d, const Row &row, float
     const bool inq = qx < d.N;
     const int qs = inq ? qx : 0;
     const int ql = q_index(d, q_add(d, row.qb, row.s2, unpack_qc(d.qc[qs])));
+    // pair symmetry: a tile none of whose q-points can hold a pair with mode A <= mode B is skipped before any load (on a
+    // mesh with N1 N2 >= 32 that is every tile whose i3 plane lies above the plane of its q_B: half of the scan)
+    if (canonical_only && !__any_sync(0xffffffffu, inq && qs <= ql)) return wp;
     const float2 *pa = d.recn + (size_t)ja0 * d.N + qs, *pb = d.recn + (size_t)jb0 * d.N + ql;   // branch-major table
     float lo[TILE], hi[TILE];
 #pragma unroll
