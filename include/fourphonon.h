@@ -156,13 +156,14 @@ int fp_list4(fp_ctx *ctx, int32_t target, int32_t channel, int32_t qp, int32_t *
 #define FP_PATH_SPLIT_SERIAL 3
 int fp_set_path(fp_ctx *ctx, int path);
 
-/* Pair symmetry of the 4ph +- and -- channels.  fp_setup checks whether the IFC4 list is invariant under the exchange of
- * its last two legs (Phi^{abgt}(i,j,k Rk,l Rl) = Phi^{abtg}(i,j,l Rl,k Rk) to 1e-13 of the largest entry: a derivative
- * symmetry of every physical force-constant set).  If it is, |V4| and the occupation factors of the +- and -- channels
- * are symmetric under lambda'' <-> lambda''', and the split path evaluates the matrix element of
- * each unordered pair once, taking the window decision (pinned arithmetic) and the Gaussian weight of both orderings
- * separately: counts stay bit-exact, rates change by summation order only.  fp_set_symmetry(ctx, 0) turns the reuse off;
- * fp_get_symmetry returns 1 if it is in effect.                                                                       */
+/* Pair symmetry of the channels whose two free legs are both conjugated: 3ph -, 4ph +- and --.  fp_setup checks whether
+ * each IFC list is invariant under the exchange of its last two legs (Phi^{abgt}(i,j,k Rk,l Rl) = Phi^{abtg}(i,j,l Rl,k Rk),
+ * resp. Phi^{abg}(i,j Rj,k Rk) = Phi^{agb}(i,k Rk,j Rj), to 1e-13 of the largest entry: a derivative symmetry of every
+ * physical force-constant set).  If it is, |V| and the occupation factors of those channels are symmetric under the
+ * exchange of the two free legs, and the split path evaluates the matrix element of each unordered
+ * pair once, taking the window decision (pinned arithmetic) and the Gaussian weight of both orderings separately: counts
+ * stay bit-exact, rates change by summation order only.  fp_set_symmetry(ctx, 0) turns the reuse off; fp_get_symmetry
+ * returns a bit mask of what is in effect: 1 = 3ph, 2 = 4ph.                                                         */
 int fp_set_symmetry(fp_ctx *ctx, int on);
 int fp_get_symmetry(const fp_ctx *ctx);
 

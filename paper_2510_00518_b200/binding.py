@@ -379,8 +379,12 @@ class Context:
         self._check(self.lib.fp_set_symmetry(self.ctx, 1 if on else 0))
 
     def get_symmetry(self) -> bool:
-        """True if fp_setup found the IFC4 list symmetric in its last two legs and the reuse is on."""
-        return self.lib.fp_get_symmetry(self.ctx) == 1
+        """True if fp_setup found an IFC list symmetric in its last two legs and the reuse is on (get_symmetry_mask: which)."""
+        return self.lib.fp_get_symmetry(self.ctx) > 0
+
+    def get_symmetry_mask(self) -> int:
+        """bit 0: 3ph - channel, bit 1: 4ph +- and -- channels"""
+        return int(self.lib.fp_get_symmetry(self.ctx))
 
     def profile_enable(self, on=True):
         self._check(self.lib.fp_profile_enable(self.ctx, 1 if on else 0))

@@ -127,34 +127,44 @@ int analyse_ifc(const fp_ifc *f, int order, int nat, const int32_t mesh[3], IfcH
     return FP_OK;
 }
 
-// Is the IFC4 list invariant under the exchange of its last two legs, Phi^{abgt}(i,j,k Rk,l Rl) = Phi^{abtg}(i,j,l Rl,k Rk)
-// (a derivative symmetry every physical force-constant set has)?  Then |V4| and the weights of the +- and -- channels
-// are symmetric under lambda'' <-> lambda''' and the split path evaluates each unordered pair
-// once.  Tolerance: 1e-13 of the largest entry.
-bool ifc4_last_legs_symmetric(const fp_ifc *f) {
-    typedef std::tuple<int, int, int, int, int, int, int, int, int, int, int, int, int> K;   // i j k l Rj Rk Rl
+// Is the IFC list invariant under the exchange of its last two legs -- Phi^{abgt}(i,j,k Rk,l Rl) = Phi^{abtg}(i,j,l Rl,k Rk)
+// for order 4, Phi^{abg}(i,j Rj,k Rk) = Phi^{agb}(i,k Rk,j Rj) for order 3 (a derivative symmetry every physical
+// force-constant set has)?  Then |V| and the weights of the channels whose two free legs are both conjugated (3ph -,
+// 4ph +- and --) are symmetric under the exchange of those legs and the split path evaluates
+// each unordered pair once.  Tolerance: 1e-13 of the largest entry.
+bool ifc_last_legs_symmetric(const fp_ifc *f, int order) {
+    typedef std::vector<int> K;                              // fixed legs, then the two exchangeable legs (atom, R)
+    const int nfix = order - 3;                              // order 4: leg j is fixed
+    const int ncomp = order == 3 ? 27 : 81, nlead = ncomp / 9;
     std::map<K, int64_t> idx;
     auto key = [&](int64_t c, bool swap) {
-        const int32_t *at = f->atoms + c * 4, *cl = f->cells + c * 9;
-        const int32_t *Rk = cl + (swap ? 6 : 3), *Rl = cl + (swap ? 3 : 6);
-        return K(at[0], at[1], swap ? at[3] : at[2], swap ? at[2] : at[3], cl[0], cl[1], cl[2], Rk[0], Rk[1], Rk[2], Rl[0], Rl[1],
-                 Rl[2]);
+        const int32_t *at = f->atoms + c * order, *cl = f->cells + c * (order - 1) * 3;
+        K k;
+        k.push_back(at[0]);
+        for (int m = 0; m < nfix; m++) { k.push_back(at[1 + m]); for (int x = 0; x < 3; x++) k.push_back(cl[3 * m + x]); }
+        const int a = order - 2, b = order - 1;              // the last two legs
+        const int32_t *Ra = cl + 3 * (a - 1), *Rb = cl + 3 * (b - 1);
+        const int la = swap ? b : a, lb = swap ? a : b;
+        const int32_t *R1 = swap ? Rb : Ra, *R2 = swap ? Ra : Rb;
+        k.push_back(at[la]); for (int x = 0; x < 3; x++) k.push_back(R1[x]);
+        k.push_back(at[lb]); for (int x = 0; x < 3; x++) k.push_back(R2[x]);
+        return k;
     };
     double big = 0.0;
     for (int64_t c = 0; c < f->n; c++) {
         if (!idx.emplace(key(c, false), c).second) return false;   // duplicate cluster: do not reason about sums, stay safe
-        for (int x = 0; x < 81; x++) big = std::max(big, std::fabs(f->phi[c * 81 + x]));
+        for (int x = 0; x < ncomp; x++) big = std::max(big, std::fabs(f->phi[c * ncomp + x]));
     }
     const double tol = 1e-13 * big;
     for (int64_t c = 0; c < f->n; c++) {
         auto it = idx.find(key(c, true));
-        const double *P = f->phi + c * 81;
+        const double *P = f->phi + c * ncomp;
         if (it == idx.end()) {                                // no partner: symmetric only if the cluster is zero
-            for (int x = 0; x < 81; x++) if (std::fabs(P[x]) > tol) return false;
+            for (int x = 0; x < ncomp; x++) if (std::fabs(P[x]) > tol) return false;
             continue;
         }
-        const double *Q = f->phi + it->second * 81;
-        for (int ab = 0; ab < 9; ab++)
+        const double *Q = f->phi + it->second * ncomp;
+        for (int ab = 0; ab < nlead; ab++)
             for (int g = 0; g < 3; g++)
                 for (int t = 0; t < 3; t++)
                     if (std::fabs(P[ab * 9 + g * 3 + t] - Q[ab * 9 + t * 3 + g]) > tol) return false;
@@ -333,11 +343,15 @@ int fp_setup(const fp_crystal *crystal, const double *masses, const double *omeg
         fail(ctx, FP_ENOMEM, "workspace too small for the mode tables"); return bail(FP_ENOMEM);
     }
     d.rec = rec; d.recf = recf; d.recn = recn; d.occ = occ; d.evec = evec; d.evecc = evecc; d.ph1d = ph1d; d.qc = qc;
-    if (ifc3) { int rc = upload_ifc(ctx, bump, h3, ctx->i3, st); if (rc) return bail(rc); ctx->has3 = true; }
+    if (ifc3) {
+        int rc = upload_ifc(ctx, bump, h3, ctx->i3, st); if (rc) return bail(rc);
+        ctx->has3 = true;
+        ctx->sym23 = ifc_last_legs_symmetric(ifc3, 3);
+    }
     if (ifc4) {
         int rc = upload_ifc(ctx, bump, h4, ctx->i4, st); if (rc) return bail(rc);
         ctx->has4 = true;
-        ctx->sym34 = ifc4_last_legs_symmetric(ifc4);
+        ctx->sym34 = ifc_last_legs_symmetric(ifc4, 4);
     }
     ctx->resident = align_up(bump.off);
 
@@ -525,7 +539,7 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
         ra.prefiltered = ctx->profiling ? stat : nullptr;
         ra.overflow = reinterpret_cast<unsigned int *>(stat + 1);
         ra.evaluated = ctx->profiling ? stat + 2 : nullptr;
-        ra.sym = (order == 4 && split && ctx->sym34 && ctx->use_sym) ? 1 : 0;
+        ra.sym = (split && ctx->use_sym && (order == 4 ? ctx->sym34 : ctx->sym23)) ? 1 : 0;
         CU(cudaMemsetAsync(stat, 0, 3 * sizeof(unsigned long long), st));
         { ProfScope p(ctx, CAT_PRE, st);
           if (order == 3) launch_pre3(d, f, d_targets, nts, pre, st); else launch_pre4(d, f, d_targets, nts, pre, st); }
@@ -700,7 +714,9 @@ int fp_set_path(fp_ctx *ctx, int path) {
 }
 
 int fp_set_symmetry(fp_ctx *ctx, int on) { if (!ctx) return FP_EINVAL; ctx->use_sym = on != 0; return FP_OK; }
-int fp_get_symmetry(const fp_ctx *ctx) { return ctx ? (ctx->sym34 && ctx->use_sym ? 1 : 0) : FP_EINVAL; }
+int fp_get_symmetry(const fp_ctx *ctx) {
+    return ctx ? ((ctx->use_sym && ctx->sym23 ? 1 : 0) | (ctx->use_sym && ctx->sym34 ? 2 : 0)) : FP_EINVAL;
+}
 
 int fp_profile_enable(fp_ctx *ctx, int on) { if (!ctx) return FP_EINVAL; ctx->profiling = on != 0; return FP_OK; }
 

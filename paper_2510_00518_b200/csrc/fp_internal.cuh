@@ -61,7 +61,8 @@ struct RowArgs {
     int qp_begin, nqp;            // 4ph only
     unsigned long long *prefiltered;   // nullable: += candidates admitted by the FP32 pre-filter (profiling)
     unsigned long long *evaluated;     // nullable: += list entries written by k_enum = matrix elements k_eval evaluates
-    int sym;                      // 1: 4ph rows of the +- and -- channels list each unordered {lambda'', lambda'''} pair once
+    int sym;                      // 1: rows whose two free legs are both conjugated (3ph -, 4ph +- and --) list each
+                                  // unordered pair of them once
     unsigned int *overflow;       // split path: += 1 for every (row, warp) list slot that filled up (the driver then
                                   // re-runs those rows through the fused kernel)
 };
@@ -81,7 +82,7 @@ struct fp_ctx {
     int sm_count = 148;
     bool profiling = false;
     int path = FP_PATH_AUTO;      // fp_set_path
-    bool sym34 = false;           // IFC4 is symmetric under the exchange of its last two legs (checked by fp_setup)
+    bool sym34 = false, sym23 = false;   // IFC4 / IFC3 is symmetric under the exchange of its last two legs (fp_setup)
     bool use_sym = true;          // fp_set_symmetry
     cudaStream_t side = nullptr;  // second stream of the split path: the enumerator of chunk k+1 runs beside the
     cudaEvent_t ev_enum[2] = {nullptr, nullptr}, ev_eval[2] = {nullptr, nullptr};   // evaluator of chunk k

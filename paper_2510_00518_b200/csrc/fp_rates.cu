@@ -549,10 +549,10 @@ __global__ void __launch_bounds__(RT, 8) k_enum(FpDev d, RowArgs ra, int64_t cap
     const Row row = make_row<ORDER>(d, ra, ra.row0 + r);
     unsigned nout = 0, nadm = 0, nproc = 0;
     bool ovf = false;                                                 // the slot filled up: the row is redone by k_rates
-    // pair symmetry (fp_set_symmetry): in the +- and -- channels (s2 < 0) the two free legs enter V4 and the weight in the
-    // same way, so only mode A <= mode B is listed; its entry carries the weights of both orderings, each with its own
+    // pair symmetry (fp_set_symmetry): in the 3ph - and the 4ph +- and -- channels (s2 < 0) the two free legs enter V and the
+    // weight in the same way, so only mode A <= mode B is listed; its entry carries the weights of both orderings, each with its own
     // window decision in the pinned arithmetic
-    const bool sym = ORDER == 4 && ra.sym && row.s2 < 0;
+    const bool sym = ra.sym && row.s2 < 0;
     if (row.valid && !row_is_empty(d, row)) {                         // item 8: zero modes are never a leg
         ListEnt *out = lists + ((size_t)r * RW + warp) * (size_t)capw;
         uint32_t *pend = pendq + warp * PCAP;
@@ -593,7 +593,7 @@ __global__ void __launch_bounds__(RT, 8) k_enum(FpDev d, RowArgs ra, int64_t cap
                     const double t = 1.0 / (sig * W);
                     const double rr = delta * (t * W);
                     double occ;
-                    if (ORDER == 3) occ = row.s2 > 0 ? (fa - fb) : (fa + fb + 1.0);
+                    if (ORDER == 3) occ = row.s2 > 0 ? (fa - fb) : (fa + fb + 1.0);   // symmetric in (A, B) for s2 < 0
                     else occ = (row.s2 > 0 ? 1.0 + fa : fa) * fb;
                     w = occ * (exp(-(rr * rr)) * t * 0.56418958354775628695);   // 1/sqrt(pi)
                     if (!ok) w = 0.0;

@@ -396,9 +396,20 @@ def test_pair_symmetry_of_the_4ph_channels(fp):
     assert e0 == p0 and e1 < 0.62 * e0                               # ++ is not reduced, +- and -- are halved
     assert np.allclose(g1, g0, rtol=1e-12, atol=1e-13 * np.abs(g0).max())
     assert np.allclose(w1, w0, rtol=1e-12, atol=1e-13 * np.abs(w0).max())
+    # the 3ph - channel (lambda' <-> lambda'') in the same way
+    r3 = {}
+    for on in (True, False):
+        with fp.Context.from_inputs(inp, scratch_bytes=256 << 20) as ctx:
+            ctx.set_path(fp.FP_PATH_SPLIT_SERIAL)
+            ctx.set_symmetry(on)
+            ctx.profile_enable(True)
+            r3[on] = ctx.rates3(inp.targets3) + (ctx.profile_get().evaluated,)
+    assert np.array_equal(r3[True][2], r3[False][2]) and r3[True][3] < 0.8 * r3[False][3]
+    assert np.allclose(r3[True][0], r3[False][0], rtol=1e-12, atol=1e-13 * np.abs(r3[False][0]).max())
+    assert np.allclose(r3[True][1], r3[False][1], rtol=1e-12, atol=1e-13 * np.abs(r3[False][1]).max())
 
 
-def test_asymmetric_ifc4_disables_the_pair_symmetry(fp):
+def test_asymmetric_ifc_disables_the_pair_symmetry(fp):
     """An IFC4 list that is not symmetric in its last two legs (one entry perturbed) must be evaluated over the full
     domain -- and still match the oracle, which never uses any symmetry."""
     inp = fp_inputs.make_tiny("diamond", mesh=(3, 3, 3))
@@ -408,5 +419,12 @@ def test_asymmetric_ifc4_disables_the_pair_symmetry(fp):
     inp.ifc4 = (a4, c4, p4)
     t = inp.targets4[7:19]
     with fp.Context.from_inputs(inp, scratch_bytes=64 << 20) as ctx:
-        assert not ctx.get_symmetry()
+        assert ctx.get_symmetry_mask() & 2 == 0 and ctx.get_symmetry_mask() & 1 == 1   # IFC3 is still symmetric
     check4(fp, inp, t)
+    a3, c3, p3 = inp.ifc3
+    p3 = p3.copy()
+    p3[5, 0 * 9 + 1 * 3 + 2] -= 0.21                                 # component (x,y,z) of one triplet
+    inp.ifc3 = (a3, c3, p3)
+    with fp.Context.from_inputs(inp, scratch_bytes=64 << 20) as ctx:
+        assert ctx.get_symmetry_mask() == 0
+    check3(fp, inp, inp.targets3[::5])
