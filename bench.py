@@ -177,6 +177,7 @@ def main():
     dev = torch.device("cuda", local)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
+    fp.build_library(force=False)          # no-op when the in-tree .so is newer than its sources (nvcc, sm_100a)
     fp.load_library()
 
     jobs = workload(args.config)

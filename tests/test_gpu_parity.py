@@ -19,6 +19,7 @@ def fp():
     if not torch.cuda.is_available():
         pytest.skip("needs a CUDA device")
     import paper_2510_00518_b200 as fp
+    fp.build_library(force=False)          # no-op when the in-tree .so is up to date
     fp.load_library()
     return fp
 
