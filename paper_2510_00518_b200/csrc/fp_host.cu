@@ -183,7 +183,7 @@ size_t ifc_resident_bytes(int64_t n, int order, int nat) {
 size_t tables_resident_bytes(int nat, const int32_t mesh[3], long L) {
     size_t N = (size_t)mesh[0] * mesh[1] * mesh[2], nb = 3 * (size_t)nat, M = N * nb;
     return align_up(M * sizeof(ModeRec)) + align_up(M * 16) + align_up(M * 8) * 2 + align_up(M * nb * 16) * 2 +
-           align_up((size_t)L * 16) + align_up(N * 4) + align_up(nat * 8) + 256 * 10;
+           align_up((size_t)L * 16) + align_up(N * 4) + align_up(N * 8) + align_up(nat * 8) + 256 * 11;
 }
 
 long mesh_lcm(const int32_t mesh[3]) {
@@ -338,11 +338,12 @@ int fp_setup(const fp_crystal *crystal, const double *masses, const double *omeg
     double2 *evecc = bump.take<double2>(M * nb);
     double2 *ph1d = bump.take<double2>(L);
     int *qc = bump.take<int>(N);
+    float2 *qmm = bump.take<float2>(N);
     double *masses_dev = bump.take<double>(nat);
-    if (!rec || !recf || !recn || !maxima || !occ || !evec || !evecc || !ph1d || !qc || !masses_dev) {
+    if (!rec || !recf || !recn || !maxima || !occ || !evec || !evecc || !ph1d || !qc || !qmm || !masses_dev) {
         fail(ctx, FP_ENOMEM, "workspace too small for the mode tables"); return bail(FP_ENOMEM);
     }
-    d.rec = rec; d.recf = recf; d.recn = recn; d.occ = occ; d.evec = evec; d.evecc = evecc; d.ph1d = ph1d; d.qc = qc;
+    d.rec = rec; d.recf = recf; d.recn = recn; d.occ = occ; d.evec = evec; d.evecc = evecc; d.ph1d = ph1d; d.qc = qc; d.qmm = qmm;
     if (ifc3) {
         int rc = upload_ifc(ctx, bump, h3, ctx->i3, st); if (rc) return bail(rc);
         ctx->has3 = true;
@@ -388,7 +389,7 @@ int fp_setup(const fp_crystal *crystal, const double *masses, const double *omeg
     // stage 1 of the FP32 pre-filter: |Delta_f| <= n'_a + n'_b with n' = cs |u| (1+1e-6) + slack
     d.pfCs = d.sigma_const > 0.0 ? 0.5 * d.ncut * d.sigma_const : d.ncut * d.scale / std::sqrt(6.0);
     d.pfSlack = 2e-6 * wmax;                                          // per leg; covers |Delta_f - Delta| and 4 FP32 adds
-    launch_tables(d, d_omega, d_eig, d_vg, masses_dev, hbar_over_kb(), rec, recf, recn, occ, evec, evecc, ph1d, qc, maxima, st);
+    launch_tables(d, d_omega, d_eig, d_vg, masses_dev, hbar_over_kb(), rec, recf, recn, occ, evec, evecc, ph1d, qc, qmm, maxima, st);
     CU(cudaGetLastError());
     unsigned long long hmax[2] = {0, 0};
     CU(cudaMemcpyAsync(hmax, maxima, sizeof(hmax), cudaMemcpyDeviceToHost, st));
@@ -413,6 +414,8 @@ int fp_setup(const fp_crystal *crystal, const double *masses, const double *omeg
         // upper bound of every entry of the stage 1 table (same formula as k_tables, rounded up once more)
         const double nmax = (d.sigma_const > 0.0 ? d.pfCs : d.pfCs * umax) * (1.0 + 2e-6) + d.pfSlack;
         d.pfNmax = std::isfinite(nmax) ? std::nextafterf((float)nmax, INFINITY) : INFINITY;
+        // stage-1 tile test: |Delta_f| <= n'_a + n'_b <= 2 nmax, plus the rounding of the three FP32 adds of the bound
+        d.pfW = std::isfinite(nmax) ? std::nextafterf((float)(2.0 * nmax + 1e-5 * wmax), INFINITY) : INFINITY;
         d.pfK1 = std::nextafterf((float)K1, INFINITY);
         d.pfC2 = std::isinf(C2) ? INFINITY : std::nextafterf((float)C2, INFINITY);
     }

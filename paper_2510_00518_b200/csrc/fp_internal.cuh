@@ -39,6 +39,8 @@ struct FpDev {
     const double2 *evecc;         // N*nb*nb conj(e~): the conjugations of step 6 are table choices, not arithmetic
     const double2 *ph1d;          // L
     const int *qc;                // N packed mesh coordinates i1 | i2<<10 | i3<<20   (N_mu <= 1024)
+    const float2 *qmm;            // N  {min, max} of the non-zero frequencies of a q-point, rounded outward to FP32
+    float pfW;                    // no pair of a q_A, q_B can pass stage 1 unless [Delta_min, Delta_max] meets [-pfW, pfW]
 };
 
 // Anharmonic list in device layout: clusters sorted by contraction block.
@@ -99,7 +101,7 @@ enum { CAT_PRE = 0, CAT_RATES, CAT_REDUCE, CAT_ENUM, CAT_N };
 // ---- kernel launchers (fp_kernels.cu) --------------------------------------------------------------------------------
 void launch_tables(const FpDev &d, const double *omega, const double *eig, const double *vg, const double *masses_dev,
                    double hbar_over_kb, ModeRec *rec, float4 *recf, float2 *recn, double *occ, double2 *evec, double2 *evecc, double2 *ph1d, int *qc,
-                   unsigned long long *maxima /*2: bits of max omega, max |B v|_2*/, cudaStream_t st);
+                   float2 *qmm, unsigned long long *maxima /*2: bits of max omega, max |B v|_2*/, cudaStream_t st);
 // fused rate kernel (fp_rates.cu)
 void launch_pre3(const FpDev &d, const IfcDev &f, const int32_t *targets, int64_t nt, double2 *mhat, cudaStream_t st);
 void launch_pre4(const FpDev &d, const IfcDev &f, const int32_t *targets, int64_t nt, double2 *t0, cudaStream_t st);

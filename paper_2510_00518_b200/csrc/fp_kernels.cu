@@ -18,7 +18,7 @@ namespace {
 // ---------------------------------------------------------------------------------------------------------------------
 __global__ void k_tables(FpDev d, const double *omega, const double *eig, const double *vg, const double *masses,
                          double hbar_over_kb, ModeRec *rec, float4 *recf, float2 *recn, double *occ, double2 *evec, double2 *evecc, double2 *ph1d,
-                         int *qc, unsigned long long *maxima) {
+                         int *qc, float2 *qmm, unsigned long long *maxima) {
     int64_t nmodes = (int64_t)d.N * d.nb;
     int64_t gid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t m = gid; m < nmodes; m += stride) {
@@ -58,6 +58,12 @@ __global__ void k_tables(FpDev d, const double *omega, const double *eig, const 
     for (int64_t q = gid; q < d.N; q += stride) {
         int i1 = (int)(q % d.N1), i2 = (int)((q / d.N1) % d.N2), i3 = (int)(q / ((int64_t)d.N1 * d.N2));
         qc[q] = i1 | (i2 << 10) | (i3 << 20);
+        float lo = CUDART_INF_F, hi = -CUDART_INF_F;                  // stage-1 tile test: frequency range of the q-point
+        for (int j = 0; j < d.nb; j++) {
+            const double w = omega[q * d.nb + j];
+            if (w != 0.0) { lo = fminf(lo, __double2float_rd(w)); hi = fmaxf(hi, __double2float_ru(w)); }
+        }
+        qmm[q] = make_float2(lo, hi);
     }
 }
 
@@ -250,9 +256,9 @@ __global__ void __launch_bounds__(256) k_fp64_probe(int iters, double a, double 
 // ---------------------------------------------------------------------------------------------------------------------
 void launch_tables(const FpDev &d, const double *omega, const double *eig, const double *vg, const double *masses_dev,
                    double hbar_over_kb, ModeRec *rec, float4 *recf, float2 *recn, double *occ, double2 *evec, double2 *evecc, double2 *ph1d, int *qc,
-                   unsigned long long *maxima, cudaStream_t st) {
+                   float2 *qmm, unsigned long long *maxima, cudaStream_t st) {
     cudaMemsetAsync(maxima, 0, 2 * sizeof(unsigned long long), st);
-    k_tables<<<592, 256, 0, st>>>(d, omega, eig, vg, masses_dev, hbar_over_kb, rec, recf, recn, occ, evec, evecc, ph1d, qc, maxima);
+    k_tables<<<592, 256, 0, st>>>(d, omega, eig, vg, masses_dev, hbar_over_kb, rec, recf, recn, occ, evec, evecc, ph1d, qc, qmm, maxima);
 }
 
 void launch_count(int order, const FpDev &d, const RowArgs &ra, int64_t nrows, uint32_t *counts, cudaStream_t st) {

@@ -364,9 +364,17 @@ __device__ __forceinline__ int stage1_step(const FpDev &d, const Row &row, float
     const bool inq = qx < d.N;
     const int qs = inq ? qx : 0;
     const int ql = q_index(d, q_add(d, row.qb, row.s2, unpack_qc(d.qc[qs])));
-    // pair symmetry: a tile none of whose q-points can hold a pair with mode A <= mode B is skipped before any load (on a
-    // mesh with N1 N2 >= 32 that is every tile whose i3 plane lies above the plane of its q_B: half of the scan)
-    if (canonical_only && !__any_sync(0xffffffffu, inq && qs <= ql)) return wp;
+    // Tile test, one warp vote before the branch records are loaded: a q-point whose frequency ranges cannot bring Delta
+    // into [-pfW, pfW] holds no stage-1 survivor (most tiles of the ++ and -- rows with a large base energy); with the
+    // pair symmetry neither does one with q_A above q_B (on a mesh with N1 N2 >= 32 every tile whose i3 plane lies above
+    // the plane of its q_B: half of the scan).
+    {
+        const float2 mA = __ldg(d.qmm + qs), mB = __ldg(d.qmm + ql);
+        const float dmin = (row.s2 > 0 ? basef + mA.x : basef - mA.y) - mB.y;
+        const float dmax = (row.s2 > 0 ? basef + mA.y : basef - mA.x) - mB.x;
+        const bool live = inq && dmin <= d.pfW && dmax >= -d.pfW && (!canonical_only || qs <= ql);
+        if (!__any_sync(0xffffffffu, live)) return wp;
+    }
     const float2 *pa = d.recn + (size_t)ja0 * d.N + qs, *pb = d.recn + (size_t)jb0 * d.N + ql;   // branch-major table
     float lo[TILE], hi[TILE];
 #pragma unroll
