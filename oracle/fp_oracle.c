@@ -19,7 +19,9 @@
  * the thread count.
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): brute-force momentum enumeration and an independent dense-Fourier
- * evaluation on 2x2x2 / 3x2x1 meshes, closed-form counts with the filter disabled, the 1-atom single-entry |V|^2 closed
+ * evaluation on 2x2x2 / 3x2x1 meshes, the adaptive-sigma window of BOTH orders against brute-force process lists on
+ * 3x3x3 / 3x2x1 / 3x3x2 meshes (3ph: sigma from v' - v''; 4ph: sigma from v'' - v''', the reading of SURVEY.md §8(c)
+ * item 2) with the weighted phase space summed directly over those lists, closed-form counts with the filter disabled, the 1-atom single-entry |V|^2 closed
  * form, gauge / cell-offset invariance, permutation symmetry of |V|, vanishing |V| for Gamma-acoustic legs under the
  * sum rule, time reversal, dyadic window-edge cases, sigma closed form on a cubic cell, on-shell occupation identities,
  * high-T scaling, kappa limits, CODATA constants derived two ways.
@@ -317,6 +319,7 @@ int orc_rates4(const orc_setup *s, const int32_t *targets, int64_t nt, int32_t q
     const double C4 = const_c4();
     static const int S1[3] = { +1, +1, -1 }, S2[3] = { +1, -1, -1 };
     const int nqp = qp_end - qp_begin;
+    if (qp_begin < 0 || qp_end > N) return -2;                               /* q' range outside the mesh */
     if (nqp <= 0) { for (int64_t i = 0; i < nt * 3; i++) { gamma[i] = 0; if (wp) wp[i] = 0; counts[i] = 0; } return 0; }
     ksum *pg = calloc((size_t)nt * nqp * 3, sizeof(ksum)), *pw = calloc((size_t)nt * nqp * 3, sizeof(ksum));
     int64_t *pc = calloc((size_t)nt * nqp * 3, sizeof(int64_t));
@@ -378,6 +381,38 @@ int orc_rates4(const orc_setup *s, const int32_t *targets, int64_t nt, int32_t q
         }
     free(pg); free(pw); free(pc);
     return 0;
+}
+
+/* process list of one target and channel over q' in [qp_begin, qp_end), as (lam1, lam2, lam3) triples in loop order:
+ * the 4ph analogue of orc_list3 -- the loop nest, the sigma legs (v'' - v''') and the filter
+ * are those of orc_rates4.  Returns the count (may exceed cap), -2 for a q' range outside the mesh.                   */
+int64_t orc_list4(const orc_setup *s, int32_t lam, int ch, int32_t qp_begin, int32_t qp_end, int32_t *triples, int64_t cap) {
+    const int nb = 3 * s->natoms, N = nq_of(s);
+    double B[9]; orc_recip(s->lattvec, s->mesh, B);
+    static const int S1[3] = { +1, +1, -1 }, S2[3] = { +1, -1, -1 };
+    if (qp_begin < 0 || qp_end > N) return -2;
+    int q = lam / nb, s1 = S1[ch], s2 = S2[ch]; double w = s->omega[lam];
+    int64_t n = 0;
+    if (w == 0.0) return 0;
+    for (int q1 = qp_begin; q1 < qp_end; q1++)
+        for (int j1 = 0; j1 < nb; j1++) {
+            int lam1 = q1 * nb + j1; double w1 = s->omega[lam1]; if (w1 == 0.0) continue;
+            for (int q2 = 0; q2 < N; q2++) {
+                int q3 = q_combine(s, q, s1, q1, s2, q2);
+                for (int j2 = 0; j2 < nb; j2++) {
+                    int lam2 = q2 * nb + j2; double w2 = s->omega[lam2]; if (w2 == 0.0) continue;
+                    for (int j3 = 0; j3 < nb; j3++) {
+                        int lam3 = q3 * nb + j3; double w3 = s->omega[lam3]; if (w3 == 0.0) continue;
+                        double sigma = sigma_of(s, B, s->vg + 3 * (size_t)lam2, s->vg + 3 * (size_t)lam3);
+                        double delta = ch == 0 ? ((w + w1) + w2) - w3 : ch == 1 ? ((w + w1) - w2) - w3 : ((w - w1) - w2) - w3;
+                        if (!allowed(s, delta, sigma)) continue;
+                        if (n < cap) { triples[3 * n] = lam1; triples[3 * n + 1] = lam2; triples[3 * n + 2] = lam3; }
+                        n++;
+                    }
+                }
+            }
+        }
+    return n;
 }
 
 /* ---- step 8: RTA thermal conductivity ---------------------------------------------------------------------------- */

@@ -51,6 +51,8 @@ def lib():
         _lib.orc_allowed.argtypes = [C.c_void_p, C.c_double, C.c_double]
         _lib.orc_list3.restype = C.c_int64
         _lib.orc_list3.argtypes = [C.c_void_p, C.c_int32, C.c_int, C.c_void_p, C.c_int64]
+        _lib.orc_list4.restype = C.c_int64
+        _lib.orc_list4.argtypes = [C.c_void_p, C.c_int32, C.c_int, C.c_int32, C.c_int32, C.c_void_p, C.c_int64]
         _lib.orc_rates3.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
         _lib.orc_rates4.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p,
                                     C.c_void_p, C.c_int]
@@ -152,6 +154,8 @@ class Oracle:
         g = np.zeros((t.size, 3)); w = np.zeros((t.size, 3)); c = np.zeros((t.size, 3), dtype=np.int64)
         rc = self.lib.orc_rates4(self.sp, _ptr(t), t.size, int(qp_begin), int(qp_end), _ptr(g), _ptr(w), _ptr(c),
                                  int(weights_only))
+        if rc == -2:
+            raise ValueError("oracle rates4: q' range outside the mesh")
         if rc != 0:
             raise MemoryError("oracle rates4")
         return g, w, c
@@ -161,6 +165,15 @@ class Oracle:
         pairs = np.zeros((max(n, 1), 2), dtype=np.int32)
         self.lib.orc_list3(self.sp, int(lam), int(ch), _ptr(pairs), n)
         return pairs[:n]
+
+    def list4(self, lam, ch, qp_begin=0, qp_end=None):
+        qp_end = self.N if qp_end is None else qp_end
+        n = self.lib.orc_list4(self.sp, int(lam), int(ch), int(qp_begin), int(qp_end), None, 0)
+        if n < 0:
+            raise ValueError("oracle list4: q' range outside the mesh")
+        tr = np.zeros((max(n, 1), 3), dtype=np.int32)
+        self.lib.orc_list4(self.sp, int(lam), int(ch), int(qp_begin), int(qp_end), _ptr(tr), n)
+        return tr[:n]
 
     def kappa(self, gamma_total):
         g = np.ascontiguousarray(gamma_total, dtype=np.float64).reshape(-1)

@@ -185,3 +185,51 @@ def rates4_bruteforce(inp, lam, sigma, T=300.0):
                                 out_c[ch] += 1
         out_g[ch] *= c4 / N ** 2 * (1.0 / 6.0 if ch == 2 else 0.5)
     return out_g, out_c
+
+
+def list4_bruteforce(inp, lam, ch, scale=1.0, ncut=2.0, T=300.0):
+    """Adaptive-sigma 4ph process list of one target and channel by brute force over ALL (q', q'', q''') triples (rational
+    momentum test), the window |Delta| <= ncut sigma with sigma = scale sqrt(sum_mu (B_mu . (v'' - v'''))^2 / 6) -- the
+    reading of SURVEY.md §8(c) item 2 / DESIGN.md §3-2: the LAST TWO legs -- in plain numpy, and the weighted phase space
+    of PAPER.md:163's Gaussian with the "/f" occupation forms (item 5).
+    -> (set of (lam1, lam2, lam3), {triple: |Delta| - ncut sigma} for edge checks, WP sum incl. the symmetry weight / N^2)"""
+    fr = frac_coords(inp)
+    nb, N = inp.nb, inp.nq
+    q = lam // nb
+    w = inp.omega.reshape(N, nb)
+    v = inp.vg.reshape(N, nb, 3)
+    Bm = recip_cart(inp.crystal.lattvec) / np.asarray(inp.mesh, float)[:, None]      # rows B_mu = b_mu / N_mu
+    s1, s2 = ((1, 1), (1, -1), (-1, -1))[ch]
+    w0 = w[q, lam % nb]
+    out, margin, wp = set(), {}, 0.0
+    if w0 == 0:
+        return out, margin, 0.0
+    f0 = be(w0, T)
+    for q1 in range(N):
+        for q2 in range(N):
+            for q3 in range(N):
+                if not conserves(fr, (q, q1, q2, q3), (1, s1, s2, -1)):
+                    continue
+                dv = v[q2][:, None, :] - v[q3][None, :, :]                        # (j2, j3, 3): v'' - v'''
+                sig = scale * np.sqrt(((dv @ Bm.T) ** 2).sum(axis=-1) / 6.0)       # (j2, j3)
+                for j1 in range(nb):
+                    w1 = w[q1, j1]
+                    if w1 == 0:
+                        continue
+                    d = w0 + s1 * w1 + s2 * w[q2][:, None] - w[q3][None, :]
+                    ok = (sig > 0) & (np.abs(d) <= ncut * sig) & (w[q2][:, None] != 0) & (w[q3][None, :] != 0)
+                    f1 = be(w1, T)
+                    for j2, j3 in zip(*np.nonzero(ok)):
+                        t = (q1 * nb + j1, q2 * nb + int(j2), q3 * nb + int(j3))
+                        out.add(t)
+                        margin[t] = abs(d[j2, j3]) - ncut * sig[j2, j3]
+                        w2, w3 = w[q2, j2], w[q3, j3]
+                        f2, f3 = be(w2, T), be(w3, T)
+                        occ = ((1 + f1) if s1 > 0 else f1) * ((1 + f2) if s2 > 0 else f2) * f3 / f0
+                        g = np.exp(-(d[j2, j3] / sig[j2, j3]) ** 2) / (sig[j2, j3] * np.sqrt(np.pi))
+                        wp += occ * g / (w0 * w1 * w2 * w3)
+                    # near misses, for the edge rule of the set comparison
+                    near = (sig > 0) & ~ok & (np.abs(np.abs(d) - ncut * sig) < 1e-9) & (w[q2][:, None] != 0) & (w[q3][None, :] != 0)
+                    for j2, j3 in zip(*np.nonzero(near)):
+                        margin[(q1 * nb + j1, q2 * nb + int(j2), q3 * nb + int(j3))] = abs(d[j2, j3]) - ncut * sig[j2, j3]
+    return out, margin, wp * (1.0 / 6.0 if ch == 2 else 0.5) / N ** 2

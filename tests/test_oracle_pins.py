@@ -328,6 +328,47 @@ def test_list3_is_momentum_conserving_and_matches_bruteforce_set():
     assert total > 50
 
 
+@pytest.mark.parametrize("kind,mesh,lams", [("diamond", (3, 3, 3), (31, 100)), ("diamond", (3, 2, 1), (8, 21)),
+                                            ("sc1", (3, 3, 2), (20,))])
+def test_list4_adaptive_sigma_matches_bruteforce_set_and_weights(kind, mesh, lams):
+    """The 4ph ADAPTIVE-sigma path (SURVEY.md §8(c) item 2 / DESIGN.md §3-2: sigma from the last two legs, v2 - v3; the
+    paper shows only compute_sigma(v1 - v2) for 3ph).  For each channel: (i) orc_list4 equals, as a set, a
+    brute-force scan over ALL (lam1, lam2, lam3) with rational momentum test and an independent numpy evaluation of
+    sigma and the window; (ii) orc_rates4's counts equal the list length; (iii) orc_rates4(weights_only) equals the
+    direct sum of PAPER.md:163's Gaussian with the "/f" occupation forms over the brute-force list.  A sigma built from
+    (v1, v2) instead, or a wrong sign of omega2 in Delta, fails (i), (ii) and (iii)."""
+    inp = fi.make_tiny(kind, mesh)
+    o = Oracle(inp)
+    total = 0
+    for lam in lams:
+        t = np.array([lam], dtype=np.int32)
+        _, wp, cnt = o.rates4(t, weights_only=True)
+        for ch in range(3):
+            want, margin, wsum = bf.list4_bruteforce(inp, lam, ch, scale=inp.scale, T=inp.T)
+            got = set(map(tuple, o.list4(lam, ch).tolist()))
+            assert len(got) == cnt[0, ch]                               # the list and the rate loop decide alike
+            # candidates within rounding of the window edge may legitimately differ between two arithmetics
+            for tr in got ^ want:
+                assert tr in margin and abs(margin[tr]) < 1e-10
+            if got == want:
+                assert wp[0, ch] == pytest.approx(wsum, rel=1e-11)
+            total += len(want)
+    assert total > 200                                                  # the adaptive window really admits processes
+
+
+def test_list4_partial_q_range_and_bounds():
+    inp = fi.make_tiny("diamond", (3, 3, 3))
+    o = Oracle(inp)
+    full = o.list4(50, 1)
+    part = np.concatenate([o.list4(50, 1, 0, 10), o.list4(50, 1, 10, 27)])
+    assert np.array_equal(full, part)                                   # loop order: q' outermost
+    assert len(np.unique(full, axis=0)) == len(full)
+    with pytest.raises(ValueError):
+        o.list4(50, 1, 0, 28)
+    with pytest.raises(ValueError):
+        o.rates4(np.array([50], dtype=np.int32), 5, 28)
+
+
 @pytest.mark.parametrize("kind,lams", [("diamond", (4, 29)), ("sc1", (5, 13, 22))])
 def test_rates3_bruteforce_2x2x2(kind, lams):
     """Full rates vs the brute-force/dense-Fourier route on 2x2x2 (constant sigma, filter off), both channels."""
