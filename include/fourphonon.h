@@ -176,6 +176,13 @@ int fp_profile_get(fp_ctx *ctx, fp_profile *out);           /* synchronises the 
  * cross-check).                                                                                       */
 int fp_probe_fp64_tflops(void *stream, double *tflops);
 
+/* FP64 tensor-core microbenchmark (the dense-recast decision is taken by measurement, north_star
+ * "only if ncu shows the gain"): mma.sync.m8n8k4.f64 (SASS DMMA.8x8x4) on all SMs, 8 independent accumulator tiles per
+ * warp.  out (HOST, 3 doubles), TFLOP/s: [0] DMMA alone, [1] DFMA alone in the same kernel shape (64 chains per thread),
+ * [2] both kinds interleaved (flops of both / time: the sum of [0] and [1] if the two kinds issue side by side, their
+ * harmonic combination if they share a pipe).                                                                        */
+int fp_probe_dmma_tflops(void *stream, double out[3]);
+
 /* Unit constants as derived inside the library from CODATA 2018: out[0]=C3, out[1]=C4 (1/ps), out[2]=C_kappa,
  * out[3]=hbar/kB (ps K).                                                                                              */
 void fp_constants(double out[4]);

@@ -28,7 +28,7 @@ _SOURCES = ["fp_kernels.cu", "fp_rates.cu", "fp_host.cu"]
 # every symbol include/fourphonon.h declares (tests check that the built library exports all of them)
 EXPORTED_SYMBOLS = [
     "fp_workspace_bytes", "fp_setup", "fp_rates3", "fp_rates4", "fp_kappa_rta", "fp_list3", "fp_list4",
-    "fp_set_path", "fp_set_symmetry", "fp_get_symmetry", "fp_profile_enable", "fp_profile_reset", "fp_profile_get", "fp_probe_fp64_tflops", "fp_constants",
+    "fp_set_path", "fp_set_symmetry", "fp_get_symmetry", "fp_profile_enable", "fp_profile_reset", "fp_profile_get", "fp_probe_fp64_tflops", "fp_probe_dmma_tflops", "fp_constants",
     "fp_last_error", "fp_version", "fp_destroy",
 ]
 
@@ -142,6 +142,8 @@ def load_library():
     lib.fp_profile_get.argtypes = [vp, C.POINTER(_Profile)]
     lib.fp_probe_fp64_tflops.restype = C.c_int
     lib.fp_probe_fp64_tflops.argtypes = [vp, C.POINTER(dbl)]
+    lib.fp_probe_dmma_tflops.restype = C.c_int
+    lib.fp_probe_dmma_tflops.argtypes = [vp, C.POINTER(dbl)]
     lib.fp_constants.restype = None
     lib.fp_constants.argtypes = [C.POINTER(dbl)]
     lib.fp_last_error.restype = C.c_char_p
@@ -178,6 +180,15 @@ def fp_probe_fp64_tflops(stream=None) -> float:
     if rc != FP_OK:
         raise FourPhononError(rc, "fp_probe_fp64_tflops failed")
     return out.value
+
+
+def fp_probe_dmma_tflops(stream=None) -> dict:
+    """TFLOP/s of DMMA.8x8x4 alone, DFMA alone and both interleaved (include/fourphonon.h)."""
+    out = (C.c_double * 3)()
+    rc = load_library().fp_probe_dmma_tflops(_stream_ptr(stream), out)
+    if rc != FP_OK:
+        raise FourPhononError(rc, "fp_probe_dmma_tflops failed")
+    return {"dmma": out[0], "dfma": out[1], "dmma_and_dfma": out[2]}
 
 
 def _is_torch(x):

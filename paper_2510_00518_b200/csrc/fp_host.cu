@@ -222,7 +222,11 @@ struct ProfScope {
     ProfScope(fp_ctx *c, int cat, cudaStream_t s) : ctx(c), st(s) {
         if (!ctx->profiling) return;
         EventRec r; r.cat = cat;
-        if (cudaEventCreate(&r.a) != cudaSuccess || cudaEventCreate(&r.b) != cudaSuccess) return;
+        cudaEvent_t *ev[2] = {&r.a, &r.b};
+        for (auto e : ev) {                                           // events are pooled across fp_profile_reset
+            if (!ctx->pool.empty()) { *e = ctx->pool.back(); ctx->pool.pop_back(); }
+            else if (cudaEventCreate(e) != cudaSuccess) return;
+        }
         cudaEventRecord(r.a, st);
         ctx->events.push_back(r);
         idx = (int)ctx->events.size() - 1;
@@ -287,7 +291,7 @@ int fp_setup(const fp_crystal *crystal, const double *masses, const double *omeg
 
     ctx = new fp_ctx();
     cudaStream_t st = (cudaStream_t)stream;
-    auto bail = [&](int code) { g_setup_err = ctx->err; if (ctx->pinned) cudaFreeHost(ctx->pinned); delete ctx; return code; };
+    auto bail = [&](int code) { g_setup_err = ctx->err; delete ctx; return code; };
 #undef CU
 #define CU(call)                                                                                         \
     do {                                                                                                 \
@@ -302,8 +306,7 @@ int fp_setup(const fp_crystal *crystal, const double *masses, const double *omeg
     CU(cudaGetDevice(&dev));
     CU(cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, dev));
     ctx->ws = (char *)workspace; ctx->ws_bytes = workspace_bytes;
-    ctx->pinned_bytes = 1 << 20;
-    CU(cudaMallocHost(&ctx->pinned, ctx->pinned_bytes));
+    ctx->device = dev;
 
     FpDev &d = ctx->d;
     d.nat = nat; d.nb = (int)nb; d.N = (int)N; d.N1 = mesh[0]; d.N2 = mesh[1]; d.N3 = mesh[2];
@@ -433,12 +436,12 @@ int fp_setup(const fp_crystal *crystal, const double *masses, const double *omeg
 int fp_destroy(fp_ctx *ctx) {
     if (!ctx) return FP_OK;
     for (auto &e : ctx->events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+    for (auto &e : ctx->pool) cudaEventDestroy(e);
     for (int i = 0; i < 2; i++) {
         if (ctx->ev_enum[i]) cudaEventDestroy(ctx->ev_enum[i]);
         if (ctx->ev_eval[i]) cudaEventDestroy(ctx->ev_eval[i]);
     }
     if (ctx->side) cudaStreamDestroy(ctx->side);
-    if (ctx->pinned) cudaFreeHost(ctx->pinned);
     delete ctx;
     return FP_OK;
 }
@@ -725,7 +728,7 @@ int fp_profile_enable(fp_ctx *ctx, int on) { if (!ctx) return FP_EINVAL; ctx->pr
 
 int fp_profile_reset(fp_ctx *ctx) {
     if (!ctx) return FP_EINVAL;
-    for (auto &e : ctx->events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+    for (auto &e : ctx->events) { ctx->pool.push_back(e.a); ctx->pool.push_back(e.b); }
     ctx->events.clear();
     ctx->prof = fp_profile{};
     return FP_OK;
@@ -760,6 +763,15 @@ int fp_probe_fp64_tflops(void *stream, double *tflops) {
     if (t <= 0) return FP_ECUDA;
     *tflops = t;
     return FP_OK;
+}
+
+int fp_probe_dmma_tflops(void *stream, double out[3]) {
+    if (!out) return FP_EINVAL;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+        return FP_ECUDA;
+    run_dmma_probe((cudaStream_t)stream, sms, out);
+    return (out[0] > 0 && out[1] > 0 && out[2] > 0) ? FP_OK : FP_ECUDA;
 }
 
 }  // extern "C"

@@ -89,11 +89,10 @@ struct fp_ctx {
     cudaStream_t side = nullptr;  // second stream of the split path: the enumerator of chunk k+1 runs beside the
     cudaEvent_t ev_enum[2] = {nullptr, nullptr}, ev_eval[2] = {nullptr, nullptr};   // evaluator of chunk k
     std::vector<EventRec> events;
-    std::vector<cudaEvent_t> pool;
+    std::vector<cudaEvent_t> pool;   // profiling events recycled by fp_profile_reset
     fp_profile prof{};
     std::string err;
-    void *pinned = nullptr;       // small pinned staging buffer
-    size_t pinned_bytes = 0;
+    int device = 0;               // the device fp_setup ran on
 };
 
 enum { CAT_PRE = 0, CAT_RATES, CAT_REDUCE, CAT_ENUM, CAT_N };
@@ -129,3 +128,4 @@ void launch_fill(int order, const FpDev &d, const RowArgs &ra, int64_t nrows, co
 void launch_decode(int order, const FpDev &d, const RowArgs &ra, const uint32_t *list, int64_t n, int32_t *out,
                    cudaStream_t st);
 double run_fp64_probe(cudaStream_t st, int sm_count);
+void run_dmma_probe(cudaStream_t st, int sm_count, double out[3]);

@@ -249,6 +249,35 @@ __global__ void __launch_bounds__(256) k_fp64_probe(int iters, double a, double 
     if (s == 123.456) out[0] = s;
 }
 
+// FP64 tensor-core probe (the DMMA decision is taken by measurement).  NM independent
+// mma.sync.m8n8k4.f64 accumulator tiles (SASS DMMA.8x8x4; the larger PTX shapes decompose into it on sm_100a) and NF
+// independent DFMA chains per thread and iteration: NM > 0, NF = 0 measures the DMMA rate, NM = 0 the DFMA rate, both > 0
+// whether the two kinds share an issue pipe (time adds up) or run side by side (time is the maximum).
+template <int NM, int NF>
+__global__ void __launch_bounds__(256) k_dmma_probe(int iters, double a, double b) {
+    double *out = &g_probe_sink;
+    double c[NM > 0 ? 2 * NM : 1], x[NF > 0 ? NF : 1];
+    const double fa = a + 1e-9 * (threadIdx.x & 3), fb = b + 1e-9 * (threadIdx.x >> 2);
+#pragma unroll
+    for (int k = 0; k < 2 * NM; k++) c[k] = threadIdx.x + k;
+#pragma unroll
+    for (int k = 0; k < NF; k++) x[k] = threadIdx.x - k;
+    for (int i = 0; i < iters; i++) {
+#pragma unroll
+        for (int k = 0; k < NM; k++)
+            asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                         : "+d"(c[2 * k]), "+d"(c[2 * k + 1]) : "d"(fa), "d"(fb));
+#pragma unroll
+        for (int k = 0; k < NF; k++) x[k] = fma(x[k], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < 2 * NM; k++) s += c[k];
+#pragma unroll
+    for (int k = 0; k < NF; k++) s += x[k];
+    if (s == 123.456) out[0] = s;
+}
+
 }  // namespace
 
 // ---------------------------------------------------------------------------------------------------------------------
@@ -323,4 +352,33 @@ double run_fp64_probe(cudaStream_t st, int sm_count) {
     }
     cudaEventDestroy(a); cudaEventDestroy(b);
     return best;
+}
+
+// -> TFLOP/s of {DMMA alone, DFMA alone (same kernel shape), both interleaved (flops of both kinds / time)}; 0 on error
+template <int NM, int NF>
+static double time_dmma_probe(cudaStream_t st, int sm_count) {
+    cudaEvent_t a, b;
+    cudaEventCreate(&a); cudaEventCreate(&b);
+    const int iters = 1 << 13, blocks = sm_count * 8;
+    k_dmma_probe<NM, NF><<<blocks, 256, 0, st>>>(256, 1.0000001, 1e-9);   // warm-up
+    double best = 0.0;
+    for (int rep = 0; rep < 5; rep++) {
+        cudaEventRecord(a, st);
+        k_dmma_probe<NM, NF><<<blocks, 256, 0, st>>>(iters, 1.0000001, 1e-9);
+        cudaEventRecord(b, st);
+        if (cudaEventSynchronize(b) != cudaSuccess) { best = 0.0; break; }
+        float ms = 0;
+        cudaEventElapsedTime(&ms, a, b);
+        // per warp and iteration: NM mma of 8x8x4 x 2 flop = 512, NF DFMA of 32 lanes x 2 flop = 64
+        const double flops = (512.0 * NM + 64.0 * NF) * (double)iters * 8.0 * (double)blocks;
+        const double tf = flops / (ms * 1e-3) * 1e-12;
+        if (tf > best) best = tf;
+    }
+    cudaEventDestroy(a); cudaEventDestroy(b);
+    return cudaGetLastError() == cudaSuccess ? best : 0.0;
+}
+void run_dmma_probe(cudaStream_t st, int sm_count, double out[3]) {
+    out[0] = time_dmma_probe<8, 0>(st, sm_count);
+    out[1] = time_dmma_probe<0, 64>(st, sm_count);
+    out[2] = time_dmma_probe<8, 64>(st, sm_count);
 }

@@ -21,6 +21,8 @@
 //   V = sum_b phi(s2 qx, dR_b) sum_{xy} Mhat_b[x][y] A(atomA_b,x) conj(e~_B(atomB_b,y)),
 // where the blocks b=(atomA,atomB,dR) merge all clusters that differ only in legs already fixed by the row, and
 // Mhat_b folds the IFC values with the fixed legs' eigenvectors and phases.  A = e~_A (s2=+) or conj(e~_A) (s2=-).
+#include <mutex>
+
 #include "fp_device.cuh"
 
 namespace {
@@ -732,12 +734,20 @@ size_t rates_smem_bytes(const FpDev &d, const IfcDev &f) {
     return (b + 15) & ~(size_t)15;
 }
 
+// Dynamic shared memory above 48 KB needs an opt-in per kernel AND per device (the attribute is a per-device setting):
+// the granted size is cached per (kernel instantiation, device), under a lock.
+struct SmemGrant { std::mutex mu; size_t granted[64] = {}; };
 template <typename K>
-static cudaError_t opt_in_smem(K kernel, size_t smem, size_t &granted) {   // opt-in limit is 227 KB minus the static part
-    if (smem > 48 * 1024 && smem > granted) {
-        cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+static cudaError_t opt_in_smem(K kernel, size_t smem, SmemGrant &g) {   // opt-in limit is 227 KB minus the static part
+    if (smem <= 48 * 1024) return cudaSuccess;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    std::lock_guard<std::mutex> lock(g.mu);
+    if (dev < 0 || dev >= 64 || smem > g.granted[dev]) {
+        e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        granted = smem;
+        if (dev >= 0 && dev < 64) g.granted[dev] = smem;
     }
     return cudaSuccess;
 }
@@ -746,7 +756,7 @@ template <int ORDER, int NAT, int TILE>
 static cudaError_t launch_rates_t(const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const double2 *pre,
                                   double2 *partial, uint32_t *counts, bool only_flagged, cudaStream_t st) {
     const size_t smem = rates_smem_bytes(d, f);
-    static size_t granted = 0;
+    static SmemGrant granted;
     cudaError_t e = opt_in_smem(k_rates<ORDER, NAT, TILE>, smem, granted);
     if (e != cudaSuccess) return e;
     k_rates<ORDER, NAT, TILE><<<(unsigned)nrows, RT, smem, st>>>(d, f, ra, pre, partial, counts, only_flagged);
@@ -799,7 +809,7 @@ static cudaError_t launch_eval_t(const FpDev &d, const IfcDev &f, const RowArgs 
                                  int64_t capw, const ListEnt *lists, const uint32_t *wcnt, const uint32_t *pcnt,
                                  double2 *partial, uint32_t *counts, cudaStream_t st) {
     const size_t smem = (tables_smem_bytes(d, f) + 15) & ~(size_t)15;
-    static size_t granted = 0;
+    static SmemGrant granted;
     cudaError_t e = opt_in_smem(k_eval<ORDER, NAT>, smem, granted);
     if (e != cudaSuccess) return e;
     k_eval<ORDER, NAT><<<(unsigned)nrows, EVT, smem, st>>>(d, f, ra, pre, capw, lists, wcnt, pcnt, partial, counts);
