@@ -23,7 +23,7 @@ FP_MEM_HOST, FP_MEM_DEVICE = 0, 1
 _PKG = Path(__file__).resolve().parent
 _CSRC = _PKG / "csrc"
 _LIB = _PKG / "libfourphonon_b200.so"
-_SOURCES = ["fp_kernels.cu", "fp_rates.cu", "fp_host.cu"]
+_SOURCES = ["fp_kernels.cu", "fp_rates.cu", "fp_group.cu", "fp_host.cu"]
 
 # every symbol include/fourphonon.h declares (tests check that the built library exports all of them)
 EXPORTED_SYMBOLS = [
@@ -46,7 +46,7 @@ def library_path() -> Path:
 def build_library(force: bool = False, verbose: bool = False) -> Path:
     """nvcc -gencode arch=compute_100a,code=sm_100a (cross-compiles without a GPU); in-tree so it ships with gpurun."""
     srcs = [_CSRC / s for s in _SOURCES]
-    deps = srcs + [_CSRC / "fp_internal.cuh", _CSRC / "fp_device.cuh", _PKG.parent / "include" / "fourphonon.h"]
+    deps = srcs + [_CSRC / "fp_internal.cuh", _CSRC / "fp_device.cuh", _CSRC / "fp_contract.cuh", _PKG.parent / "include" / "fourphonon.h"]
     if not force and _LIB.exists() and all(_LIB.stat().st_mtime >= d.stat().st_mtime for d in deps):
         return _LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
@@ -54,6 +54,8 @@ def build_library(force: bool = False, verbose: bool = False) -> Path:
            "-Xcompiler", "-fPIC,-ffp-contract=off", "-shared", "-o", str(_LIB)] + [str(s) for s in srcs]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
+    extra = os.environ.get("FP_NVCC_EXTRA", "").split()               # tuning experiments: -D knobs of the kernels
+    cmd[1:1] = extra
     subprocess.run(cmd, check=True)
     return _LIB
 

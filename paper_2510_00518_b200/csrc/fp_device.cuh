@@ -41,7 +41,9 @@ __device__ __forceinline__ int3 premul(const FpDev &d, int3 c) { return make_int
 #endif
 // 32 bytes at a 32-byte aligned address through the read-only path: one request per sector instead of two
 __device__ __forceinline__ void ldg256(const void *p, double2 &lo, double2 &hi) {
-#if FP_LDG256
+#if FP_LDG256 && defined(FP_LDG_VOLATILE)
+    asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(lo.x), "=d"(lo.y), "=d"(hi.x), "=d"(hi.y) : "l"(p));
+#elif FP_LDG256
     asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(lo.x), "=d"(lo.y), "=d"(hi.x), "=d"(hi.y) : "l"(p));
 #else
     lo = __ldg(reinterpret_cast<const double2 *>(p)); hi = __ldg(reinterpret_cast<const double2 *>(p) + 1);

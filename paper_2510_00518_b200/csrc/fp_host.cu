@@ -14,6 +14,9 @@
 #ifndef FP_SLOT_DIV
 #define FP_SLOT_DIV 4        // list slot = 1/FP_SLOT_DIV of the candidates a warp can meet
 #endif
+#ifndef FP_EVAL_TILE_BYTES
+#define FP_EVAL_TILE_BYTES (16 * 1024)   // Mhat tables of the rows of one evaluator tile (k_eval_g)
+#endif
 
 namespace {
 
@@ -182,8 +185,8 @@ size_t ifc_resident_bytes(int64_t n, int order, int nat) {
 
 size_t tables_resident_bytes(int nat, const int32_t mesh[3], long L) {
     size_t N = (size_t)mesh[0] * mesh[1] * mesh[2], nb = 3 * (size_t)nat, M = N * nb;
-    return align_up(M * sizeof(ModeRec)) + align_up(M * 16) + align_up(M * 8) * 2 + align_up(M * nb * 16) * 2 +
-           align_up((size_t)L * 16) + align_up(N * 4) + align_up(N * 8) + align_up(nat * 8) + 256 * 11;
+    return align_up(M * sizeof(ModeRec)) + align_up(M * 16) * 2 + align_up(M * 8) * 2 + align_up(M * nb * 16) * 2 +
+           align_up((size_t)L * 16) + align_up(N * 4) + align_up(N * 8) + align_up(nat * 8) + 256 * 12;
 }
 
 long mesh_lcm(const int32_t mesh[3]) {
@@ -337,16 +340,17 @@ int fp_setup(const fp_crystal *crystal, const double *masses, const double *omeg
     float2 *recn = bump.take<float2>(M);
     unsigned long long *maxima = bump.take<unsigned long long>(2);
     double *occ = bump.take<double>(M);
+    double2 *aux = bump.take<double2>(M);
     double2 *evec = bump.take<double2>(M * nb);
     double2 *evecc = bump.take<double2>(M * nb);
     double2 *ph1d = bump.take<double2>(L);
     int *qc = bump.take<int>(N);
     float2 *qmm = bump.take<float2>(N);
     double *masses_dev = bump.take<double>(nat);
-    if (!rec || !recf || !recn || !maxima || !occ || !evec || !evecc || !ph1d || !qc || !qmm || !masses_dev) {
+    if (!rec || !recf || !recn || !maxima || !occ || !aux || !evec || !evecc || !ph1d || !qc || !qmm || !masses_dev) {
         fail(ctx, FP_ENOMEM, "workspace too small for the mode tables"); return bail(FP_ENOMEM);
     }
-    d.rec = rec; d.recf = recf; d.recn = recn; d.occ = occ; d.evec = evec; d.evecc = evecc; d.ph1d = ph1d; d.qc = qc; d.qmm = qmm;
+    d.rec = rec; d.recf = recf; d.recn = recn; d.occ = occ; d.aux = aux; d.evec = evec; d.evecc = evecc; d.ph1d = ph1d; d.qc = qc; d.qmm = qmm;
     if (ifc3) {
         int rc = upload_ifc(ctx, bump, h3, ctx->i3, st); if (rc) return bail(rc);
         ctx->has3 = true;
@@ -392,7 +396,7 @@ int fp_setup(const fp_crystal *crystal, const double *masses, const double *omeg
     // stage 1 of the FP32 pre-filter: |Delta_f| <= n'_a + n'_b with n' = cs |u| (1+1e-6) + slack
     d.pfCs = d.sigma_const > 0.0 ? 0.5 * d.ncut * d.sigma_const : d.ncut * d.scale / std::sqrt(6.0);
     d.pfSlack = 2e-6 * wmax;                                          // per leg; covers |Delta_f - Delta| and 4 FP32 adds
-    launch_tables(d, d_omega, d_eig, d_vg, masses_dev, hbar_over_kb(), rec, recf, recn, occ, evec, evecc, ph1d, qc, qmm, maxima, st);
+    launch_tables(d, d_omega, d_eig, d_vg, masses_dev, hbar_over_kb(), rec, recf, recn, occ, aux, evec, evecc, ph1d, qc, qmm, maxima, st);
     CU(cudaGetLastError());
     unsigned long long hmax[2] = {0, 0};
     CU(cudaMemcpyAsync(hmax, maxima, sizeof(hmax), cudaMemcpyDeviceToHost, st));
@@ -421,6 +425,24 @@ int fp_setup(const fp_crystal *crystal, const double *masses, const double *omeg
         d.pfW = std::isfinite(nmax) ? std::nextafterf((float)(2.0 * nmax + 1e-5 * wmax), INFINITY) : INFINITY;
         d.pfK1 = std::nextafterf((float)K1, INFINITY);
         d.pfC2 = std::isinf(C2) ? INFINITY : std::nextafterf((float)C2, INFINITY);
+        // group path (k_enum_g): a pair (A, B) can hold an allowed process of a row only if the row's base energy lies
+        // within bnd = gfC |u_a - u_b|_f + gfD of omega_B - s2 omega_A, all in FP32:
+        //   ncut sigma = cs r,  r <= r_f + 2e-6 u_max (FP32 rounding of u, the subtraction, the squares, sqrt),
+        //   the FP32 interval test is off by at most 8 eps omega_max + eps bnd < 1e-6 omega_max
+        // (factors 1 + 1e-5: FP32 evaluation of the bound itself).
+        const double cs = d.sigma_const > 0.0 ? 0.0 : d.ncut * d.scale / std::sqrt(6.0);
+        const double half = d.sigma_const > 0.0 ? d.ncut * d.sigma_const * (1.0 + 1e-6) : 0.0;
+        const double gd = (half + 1e-6 * omax + cs * 2e-6 * umax) * (1.0 + 1e-5);
+        if (std::isfinite(cs) && std::isfinite(gd) && cs < 1e30 && gd < 1e30) {
+            d.gfC = std::nextafterf((float)(cs * (1.0 + 1e-5)), INFINITY);
+            d.gfD = std::nextafterf((float)gd, INFINITY);
+            const double wmx = (double)d.gfC * 2.0 * umax * (1.0 + 1e-5) + (double)d.gfD + 1e-5 * omax;
+            d.gfW = std::nextafterf((float)wmx, INFINITY);
+        } else {                                                      // ncut = inf: every pair can hold every row
+            d.gfC = 0.0f; d.gfD = INFINITY; d.gfW = INFINITY;
+        }
+        d.thrC = d.ncut * d.scale / std::sqrt(6.0);
+        d.invC = d.sigma_const > 0.0 ? 1.0 / d.sigma_const : std::sqrt(6.0) / d.scale;
     }
     *out = ctx;
     return FP_OK;
@@ -487,22 +509,30 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
 
     // ---- scratch budget: per-target arrays for a super-chunk of targets ------------------------------------------------
     const size_t scratch_all = ctx->ws_bytes - ctx->resident;
-    // ---- path: split (lists in the scratch) when half of the scratch holds two list buffers of a few hundred rows ------
-    // list slot of one (row, warp): a quarter of what can never overflow (but at least 2048 entries); a slot that fills
-    // up is flagged by k_enum and its row is redone through the fused kernel (rows of the many-branch config 4, where
-    // the +- channel admits 10 % and more of the candidates; never on the diamond configs)
+    // ---- path: group path (lists in the scratch) when half of the scratch holds the list slots of a few hundred rows ----
+    // list slot of one (row, warp): a quarter of what can never overflow (but at least 2048 entries); a group with a
+    // slot that fills up is flagged by k_enum_g and its rows are redone through the fused kernel (rows of the many-branch
+    // config 4, where the +- channel admits 10 % and more of the candidates; never on the diamond configs)
     const int64_t capw_all = enum_slot_entries(d);
     const int64_t capw = std::min(capw_all, std::max<int64_t>(((capw_all / FP_SLOT_DIV) + 31) & ~(int64_t)31, 2048));
-    const size_t row_list_bytes = (size_t)enum_warps_per_row() * ((size_t)capw * sizeof(ListEnt) + 2 * sizeof(uint32_t));
-    // FP_PATH_SPLIT runs the enumerator of chunk k+1 beside the evaluator of chunk k (two list buffers, two streams);
-    // FP_PATH_SPLIT_SERIAL -- what FP_PATH_AUTO picks -- runs them back to back through one buffer of twice the rows.
+    const size_t row_list_bytes = (size_t)enum_units(d) * ((size_t)capw * sizeof(ListEnt) + sizeof(uint32_t));
+    // Groups (fp_group.cu): targets of a super-chunk that share their q-point; the rows of a group CTA share one scan of
+    // the two free legs.  An unbounded window (ncut = inf) queues every (pair, row): small groups keep the queue bounded.
+    const size_t list_region = scratch_all / 2;
     const bool overlap = ctx->path == FP_PATH_SPLIT;
     const int nbuf = overlap ? 2 : 1;
-    int64_t chunk_rows = (int64_t)std::min<size_t>((scratch_all / 2) / (nbuf * row_list_bytes), (size_t)1 << 20);
+    const int64_t rows_fit = (int64_t)(list_region / (nbuf * row_list_bytes));   // rows whose list slots fit one buffer
+    // the queue of a warp holds FP_ENUM_QC survivors; an unbounded window (ncut = inf) queues every (pair, row)
+    const int rcap = (int)std::max<int64_t>(1, std::min<int64_t>(std::isfinite(d.gfW) ? FP_GROUP_RMAX : 4, rows_fit));
+    const int mcap = order == 3 ? std::min(rcap, d.nb) : std::max(1, rcap / d.nb);   // members (targets) of a group
+    const int njcap = order == 3 ? 1 : std::min(rcap, d.nb);        // j' of a 4ph group (all of them unless memory is short)
+    const int rbound = order == 3 ? mcap : mcap * njcap;             // rows of a group, at most
+    // FP_PATH_SPLIT runs the enumerator of chunk k+1 beside the evaluator of chunk k (two list buffers, two streams);
+    // FP_PATH_SPLIT_SERIAL -- what FP_PATH_AUTO picks -- runs them back to back through one buffer of twice the groups.
     const int64_t rows_wanted = std::min<int64_t>(nt * nch * rows_per_unit, 256);
     bool split = ctx->path == FP_PATH_SPLIT || ctx->path == FP_PATH_SPLIT_SERIAL ||
-                 (ctx->path == FP_PATH_AUTO && chunk_rows >= rows_wanted);
-    if (split && chunk_rows < 1) return fail(ctx, FP_ENOMEM, "workspace scratch too small for the process lists of one row");
+                 (ctx->path == FP_PATH_AUTO && rows_fit >= rows_wanted);
+    if (split && rows_fit < 1) return fail(ctx, FP_ENOMEM, "workspace scratch too small for the process lists of one row");
     if (split && !ctx->side) {
         int prio_lo = 0, prio_hi = 0;                                // enumerator CTAs take freed SM slots first: they need
         CU(cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi));    // few registers and keep the evaluator fed
@@ -512,9 +542,19 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
             CU(cudaEventCreateWithFlags(&ctx->ev_eval[i], cudaEventDisableTiming));
         }
     }
-    const size_t scratch = split ? scratch_all - nbuf * (size_t)chunk_rows * row_list_bytes - 4096 : scratch_all;
+    // rows of one evaluator tile: their Mhat tables share the CTA's shared memory (FP_EVAL_TILE_BYTES of it)
+    int ge = 1;
+    if (split) {
+        const size_t rowbytes = (size_t)f.nblk * 9 * sizeof(double2);
+        ge = (int)std::max<size_t>(1, std::min<size_t>((size_t)rbound, FP_EVAL_TILE_BYTES / rowbytes));
+        if (order == 4 && ge >= njcap) ge = ge / njcap * njcap;      // whole targets: their rows share the level-0 loads
+        if (eval_smem_bytes(d, f, ge) > 227 * 1024 - 1024)
+            return fail(ctx, FP_ENOMEM, "IFC block table exceeds the shared memory of one SM");
+    }
+    const size_t scratch = split ? scratch_all - list_region - 4096 : scratch_all;
     const size_t pre_per_target = (order == 3 ? (size_t)f.nblk * 9 : (size_t)f.n * 27) * sizeof(double2);
-    const size_t per_target = pre_per_target + (size_t)rows_per_target * (4 + 16) + (size_t)nch * 24 + 4 + 64;
+    const size_t per_target = pre_per_target + (size_t)rows_per_target * (4 + 16) + (size_t)nch * 24 + 4 + 64 + 16 +
+                              (order == 4 ? (size_t)d.nb * 16 : 16);   // (+ group descriptors)
     const size_t fixed = 16 * 1024;
     if (scratch < fixed + per_target) return fail(ctx, FP_ENOMEM, "workspace scratch too small for one target");
     int64_t nts_max = (int64_t)std::min<size_t>((size_t)nt, (scratch - fixed) / per_target);
@@ -536,7 +576,7 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
         double2 *pre = sc.take<double2>(nts * (pre_per_target / sizeof(double2)));
         uint32_t *cnt = sc.take<uint32_t>(nrows);
         double2 *partial = sc.take<double2>(nrows);
-        unsigned long long *stat = sc.take<unsigned long long>(3);    // [0] pre-filter survivors, [1] list overflows, [2] list entries
+        unsigned long long *stat = sc.take<unsigned long long>(5);    // [0] pre-filter survivors, [1] list overflows, [2] list entries, [3], [4] work counters
         double *o_gamma = sc.take<double>(nts * nch), *o_wp = sc.take<double>(nts * nch);
         int64_t *o_cnt = sc.take<int64_t>(nts * nch);
         if (!pre || !cnt || !partial || !stat || !o_gamma || !o_wp || !o_cnt) return fail(ctx, FP_ENOMEM, "scratch");
@@ -545,51 +585,85 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
         ra.prefiltered = ctx->profiling ? stat : nullptr;
         ra.overflow = reinterpret_cast<unsigned int *>(stat + 1);
         ra.evaluated = ctx->profiling ? stat + 2 : nullptr;
-        ra.sym = (split && ctx->use_sym && (order == 4 ? ctx->sym34 : ctx->sym23)) ? 1 : 0;
+        ra.sym = 0;
+        const int use_sym = (split && ctx->use_sym && (order == 4 ? ctx->sym34 : ctx->sym23)) ? 1 : 0;
         CU(cudaMemsetAsync(stat, 0, 3 * sizeof(unsigned long long), st));
         { ProfScope p(ctx, CAT_PRE, st);
           if (order == 3) launch_pre3(d, f, d_targets, nts, pre, st); else launch_pre4(d, f, d_targets, nts, pre, st); }
         CU(cudaGetLastError());
+        // groups: the targets of this super-chunk sorted by q-point (stable), cut where q changes or at mcap members
+        std::vector<int4> hgd;
+        std::vector<int32_t> hgmem(nts);
         if (!split) {
             ProfScope p(ctx, CAT_RATES, st);
             CU(launch_rates(order, d, f, ra, nrows, pre, partial, cnt, false, st));
         } else {
-            // chunks of rows through two list buffers: the enumerator of chunk k+1 (side stream) runs beside the evaluator
-            // of chunk k (caller's stream); buffer b is rewritten only after the evaluator that read it has finished
+            int rmaxg = 1;
+            {
+                std::vector<int32_t> ord(nts);
+                for (int64_t i = 0; i < nts; i++) ord[i] = (int32_t)i;
+                std::stable_sort(ord.begin(), ord.end(), [&](int32_t x, int32_t y) { return ht[t0 + x] / d.nb < ht[t0 + y] / d.nb; });
+                for (int64_t i = 0; i < nts; i++) hgmem[i] = ord[i];
+                for (int64_t i = 0; i < nts;) {
+                    const int32_t q = ht[t0 + ord[i]] / d.nb;
+                    int64_t e = i + 1;
+                    while (e < nts && e - i < mcap && ht[t0 + ord[e]] / d.nb == q) e++;
+                    if (order == 3) hgd.push_back(make_int4(q, (int)i, (int)(e - i), 0 | (1 << 16)));
+                    else
+                        for (int j0 = 0; j0 < d.nb; j0 += njcap)
+                            hgd.push_back(make_int4(q, (int)i, (int)(e - i), j0 | (std::min(njcap, d.nb - j0) << 16)));
+                    rmaxg = std::max<int>(rmaxg, (int)(e - i) * (order == 3 ? 1 : njcap));
+                    i = e;
+                }
+            }
+            const int64_t ng = (int64_t)hgd.size();
+            int4 *d_gd = sc.take<int4>(ng);
+            int32_t *d_gmem = sc.take<int32_t>(nts);
+            if (!d_gd || !d_gmem) return fail(ctx, FP_ENOMEM, "scratch (groups)");
+            CU(cudaMemcpyAsync(d_gd, hgd.data(), ng * sizeof(int4), cudaMemcpyHostToDevice, st));
+            CU(cudaMemcpyAsync(d_gmem, hgmem.data(), nts * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+            GroupArgs ga; ga.targets = d_targets; ga.gdesc = d_gd; ga.gmem = d_gmem;
+            ga.ng = (int)ng; ga.rmaxg = rmaxg; ga.nu = enum_units(d); ga.qp_begin = qp_begin; ga.nqp = (int)nqp; ga.gid0 = 0; ga.sym = use_sym;
+            ga.prefiltered = ra.prefiltered; ga.evaluated = ra.evaluated; ga.overflow = ra.overflow;
+            const int64_t ngc = ng * nch * nqp;                       // group CTAs: (group, channel[, q'])
+            const int64_t chunk_gc = std::min<int64_t>(ngc, (int64_t)(list_region / (nbuf * (size_t)rmaxg * row_list_bytes)));
+            const int ge_t = std::min(ge, rmaxg);
+            // chunks of group CTAs through one or two list buffers: with two, the enumerator of chunk k+1 (side stream) runs
+            // beside the evaluator of chunk k (caller's stream); buffer b is rewritten only after the evaluator that read it
+            // has finished
             ListEnt *lists[2]; uint32_t *wcnt[2];
             for (int b = 0; b < nbuf; b++) {
-                lists[b] = sc.take<ListEnt>((size_t)chunk_rows * enum_warps_per_row() * capw);
-                wcnt[b] = sc.take<uint32_t>(2 * (size_t)chunk_rows * enum_warps_per_row());   // entries, then processes
+                lists[b] = sc.take<ListEnt>((size_t)chunk_gc * rmaxg * enum_units(d) * capw);
+                wcnt[b] = sc.take<uint32_t>((size_t)chunk_gc * rmaxg * enum_units(d));
                 if (!lists[b] || !wcnt[b]) return fail(ctx, FP_ENOMEM, "scratch (process lists)");
             }
             cudaStream_t es = overlap ? ctx->side : st;
-            if (overlap) {                                           // targets and statistics are ready on st
+            if (overlap) {                                           // targets, groups and statistics are ready on st
                 CU(cudaEventRecord(ctx->ev_eval[0], st));
                 CU(cudaStreamWaitEvent(es, ctx->ev_eval[0], 0));
             }
             int k = 0;
-            for (int64_t r0 = 0; r0 < nrows; r0 += chunk_rows, k++) {
-                const int64_t nr = std::min(chunk_rows, nrows - r0);
+            for (int64_t g0 = 0; g0 < ngc; g0 += chunk_gc, k++) {
+                const int64_t n = std::min(chunk_gc, ngc - g0);
                 const int b = overlap ? (k & 1) : 0;
-                RowArgs rc = ra; rc.row0 = r0;
+                GroupArgs gc = ga; gc.gid0 = g0;
                 if (overlap && k >= 2) CU(cudaStreamWaitEvent(es, ctx->ev_eval[b], 0));
                 { ProfScope p(ctx, CAT_ENUM, es);
-                  CU(launch_enum(order, d, rc, nr, capw, lists[b], wcnt[b], wcnt[b] + chunk_rows * enum_warps_per_row(), es)); }
+                  CU(launch_enum_g(order, d, gc, n, capw, lists[b], wcnt[b], reinterpret_cast<unsigned int *>(stat + 3 + b), ctx->sm_count, es)); }
                 if (overlap) {
                     CU(cudaEventRecord(ctx->ev_enum[b], es));
                     CU(cudaStreamWaitEvent(st, ctx->ev_enum[b], 0));
                 }
                 { ProfScope p(ctx, CAT_RATES, st);
-                  CU(launch_eval(order, d, f, rc, nr, pre, capw, lists[b], wcnt[b], wcnt[b] + chunk_rows * enum_warps_per_row(),
-                                 partial + r0, cnt + r0, st)); }
+                  CU(launch_eval_g(order, d, f, gc, n, pre, capw, lists[b], wcnt[b], ge_t, partial, cnt, st)); }
                 if (overlap) CU(cudaEventRecord(ctx->ev_eval[b], st));
             }
             unsigned long long novf = 0;
             CU(cudaMemcpyAsync(&novf, stat + 1, sizeof(novf), cudaMemcpyDeviceToHost, st));
             CU(cudaStreamSynchronize(st));
-            if (novf != 0) {                                         // some list slots filled up: k_eval marked their rows in
-                ctx->prof.list_overflows += (int64_t)novf;           // cnt; redo those with the lists in shared memory
-                RowArgs rr = ra; rr.prefiltered = nullptr;
+            if (novf != 0) {                                         // some groups gave up (a list slot or the survivor queue
+                ctx->prof.list_overflows += (int64_t)novf;           // filled up): k_eval_g marked their rows in cnt; redo those
+                RowArgs rr = ra; rr.prefiltered = nullptr;           // with the lists in shared memory
                 ProfScope p(ctx, CAT_RATES, st);
                 CU(launch_rates(order, d, f, rr, nrows, pre, partial, cnt, true, st));
             }

@@ -8,6 +8,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -41,6 +42,11 @@ struct FpDev {
     const int *qc;                // N packed mesh coordinates i1 | i2<<10 | i3<<20   (N_mu <= 1024)
     const float2 *qmm;            // N  {min, max} of the non-zero frequencies of a q-point, rounded outward to FP32
     float pfW;                    // no pair of a q_A, q_B can pass stage 1 unless [Delta_min, Delta_max] meets [-pfW, pfW]
+    // group path (fp_group.cu): one FP32 interval test per (A, B) pair, then the pinned decision
+    const double2 *aux;           // N*nb  {f_lambda, 1/omega_lambda} (0, 0 for zero modes): the weight reads both together
+    float gfC, gfD;               // window half-width bound of a pair: bnd = gfC * |u_a - u_b|_f + gfD
+    float gfW;                    // upper bound of bnd over all pairs (tile vote)
+    double thrC, invC;            // ncut*scale/sqrt(6) and sqrt(6)/scale: fast path of the decision and 1/sigma
 };
 
 // Anharmonic list in device layout: clusters sorted by contraction block.
@@ -69,8 +75,25 @@ struct RowArgs {
                                   // re-runs those rows through the fused kernel)
 };
 
+// Group path: the targets of a super-chunk that share their q-point form a group; the rows of a group CTA -- 3ph:
+// (member, channel); 4ph: (member, channel, q', j') for all j' -- share q_base, hence the momentum map q_A -> q_B and
+// every record the enumerator loads, and differ only in their base energy.
+struct GroupArgs {
+    const int32_t *targets;       // device: the super-chunk's targets (local index t)
+    const int4 *gdesc;            // ng     {q-point, first member (offset into gmem), members, j'_0 | n_j' << 16}: the rows of
+                                  //        a 4ph group are (member, j') for j' in [j'_0, j'_0 + n_j')
+    const int32_t *gmem;          // local target indices, grouped
+    int ng, rmaxg;                // groups; largest row count of a group (stride of the list slots)
+    int nu;                       // enumeration units per group CTA = list slots per row (enum_units())
+    int qp_begin, nqp;            // 4ph only
+    int64_t gid0;                 // first group CTA ((g, ch) for 3ph, (g, ch, q') for 4ph) of this launch
+    int sym;                      // pair symmetry, as RowArgs::sym
+    unsigned long long *prefiltered, *evaluated;   // nullable statistics (see RowArgs)
+    unsigned int *overflow;
+};
+
 // One allowed process of a row in the split path: both free legs and the row-independent part of its weight.
-struct __align__(16) ListEnt { uint32_t x, y; double w; };   // x = qA << 6 | jA,  y = qB << 6 | jB
+struct __align__(16) ListEnt { uint32_t x, y; double w; };   // x = qA << 6 | jA (bit 31: both orderings of the pair passed),  y = qB << 6 | jB
 
 struct EventRec { int cat; cudaEvent_t a, b; };
 
@@ -99,7 +122,7 @@ enum { CAT_PRE = 0, CAT_RATES, CAT_REDUCE, CAT_ENUM, CAT_N };
 
 // ---- kernel launchers (fp_kernels.cu) --------------------------------------------------------------------------------
 void launch_tables(const FpDev &d, const double *omega, const double *eig, const double *vg, const double *masses_dev,
-                   double hbar_over_kb, ModeRec *rec, float4 *recf, float2 *recn, double *occ, double2 *evec, double2 *evecc, double2 *ph1d, int *qc,
+                   double hbar_over_kb, ModeRec *rec, float4 *recf, float2 *recn, double *occ, double2 *aux, double2 *evec, double2 *evecc, double2 *ph1d, int *qc,
                    float2 *qmm, unsigned long long *maxima /*2: bits of max omega, max |B v|_2*/, cudaStream_t st);
 // fused rate kernel (fp_rates.cu)
 void launch_pre3(const FpDev &d, const IfcDev &f, const int32_t *targets, int64_t nt, double2 *mhat, cudaStream_t st);
@@ -108,15 +131,18 @@ void launch_pre4(const FpDev &d, const IfcDev &f, const int32_t *targets, int64_
 cudaError_t launch_rates(int order, const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const double2 *pre,
                          double2 *partial, uint32_t *counts, bool only_flagged, cudaStream_t st);
 size_t rates_smem_bytes(const FpDev &d, const IfcDev &f);
-// split path (fp_rates.cu): enumerator -> process lists in the scratch -> evaluator
+// group path (fp_group.cu): group enumerator -> per-row process lists in the scratch -> tile evaluator
+#define FP_GROUP_RMAX 64          // rows of one enumerator group (they share the scan of the two free legs)
 int64_t enum_slot_entries(const FpDev &d);        // entries of one (row, warp) list slot that can never overflow
-int enum_warps_per_row();
-// wcnt[row*RW + warp] = list entries written, pcnt[row*RW + warp] = allowed processes they stand for
-cudaError_t launch_enum(int order, const FpDev &d, const RowArgs &ra, int64_t nrows, int64_t capw, ListEnt *lists,
-                        uint32_t *wcnt, uint32_t *pcnt, cudaStream_t st);
-cudaError_t launch_eval(int order, const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const double2 *pre,
-                        int64_t capw, const ListEnt *lists, const uint32_t *wcnt, const uint32_t *pcnt, double2 *partial,
-                        uint32_t *counts, cudaStream_t st);
+int enum_units(const FpDev &d);                   // enumeration units per group CTA = list slots per row
+size_t eval_smem_bytes(const FpDev &d, const IfcDev &f, int ge);   // dynamic shared memory of an evaluator tile of ge rows
+// wcnt[(group CTA * rmaxg + row-in-group) * units + unit] = list entries written (0xffffffff: the slot filled up);
+// work: a device counter the launcher zeroes (the units are dealt to the warps of a persistent grid)
+cudaError_t launch_enum_g(int order, const FpDev &d, const GroupArgs &ga, int64_t ngc, int64_t capw, ListEnt *lists,
+                          uint32_t *wcnt, unsigned int *work, int sm_count, cudaStream_t st);
+cudaError_t launch_eval_g(int order, const FpDev &d, const IfcDev &f, const GroupArgs &ga, int64_t ngc, const double2 *pre,
+                          int64_t capw, const ListEnt *lists, const uint32_t *wcnt, int ge, double2 *partial,
+                          uint32_t *counts, cudaStream_t st);
 void launch_finalize(int order, const FpDev &d, int64_t nt, int64_t rows_per_unit, const double2 *partial,
                      const uint32_t *counts, double c_over_n, double *gamma, double *wp, int64_t *cnt, cudaStream_t st);
 void launch_kappa(const FpDev &d, const double *gamma_total, double pref, double *kappa, cudaStream_t st);
@@ -129,3 +155,21 @@ void launch_decode(int order, const FpDev &d, const RowArgs &ra, const uint32_t 
                    cudaStream_t st);
 double run_fp64_probe(cudaStream_t st, int sm_count);
 void run_dmma_probe(cudaStream_t st, int sm_count, double out[3]);
+
+// Dynamic shared memory above 48 KB needs an opt-in per kernel AND per device (the attribute is a per-device setting):
+// the granted size is cached per (kernel instantiation, device), under a lock.
+struct SmemGrant { std::mutex mu; size_t granted[64] = {}; };
+template <typename K>
+static inline cudaError_t opt_in_smem(K kernel, size_t smem, SmemGrant &g) {   // opt-in limit is 227 KB minus the static part
+    if (smem <= 48 * 1024) return cudaSuccess;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    std::lock_guard<std::mutex> lock(g.mu);
+    if (dev < 0 || dev >= 64 || smem > g.granted[dev]) {
+        e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        if (dev >= 0 && dev < 64) g.granted[dev] = smem;
+    }
+    return cudaSuccess;
+}

@@ -17,7 +17,7 @@ namespace {
 // a1 / a4: resident tables
 // ---------------------------------------------------------------------------------------------------------------------
 __global__ void k_tables(FpDev d, const double *omega, const double *eig, const double *vg, const double *masses,
-                         double hbar_over_kb, ModeRec *rec, float4 *recf, float2 *recn, double *occ, double2 *evec, double2 *evecc, double2 *ph1d,
+                         double hbar_over_kb, ModeRec *rec, float4 *recf, float2 *recn, double *occ, double2 *aux, double2 *evec, double2 *evecc, double2 *ph1d,
                          int *qc, float2 *qmm, unsigned long long *maxima) {
     int64_t nmodes = (int64_t)d.N * d.nb;
     int64_t gid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x, stride = (int64_t)gridDim.x * blockDim.x;
@@ -27,6 +27,7 @@ __global__ void k_tables(FpDev d, const double *omega, const double *eig, const 
         rec[m] = r;
         double x = hbar_over_kb * w / d.T;                          // PAPER.md:151  f = 1/(exp(x)-1)
         occ[m] = (w == 0.0) ? 0.0 : 1.0 / expm1(x);
+        aux[m] = (w == 0.0) ? make_double2(0.0, 0.0) : make_double2(1.0 / expm1(x), 1.0 / w);
         // FP32 pre-filter record: u_mu = B_mu . v (so that sigma^2 = scale^2 |u_a - u_b|^2 / 6)
         double u0 = d.B[0] * r.vx + d.B[1] * r.vy + d.B[2] * r.vz;
         double u1 = d.B[3] * r.vx + d.B[4] * r.vy + d.B[5] * r.vz;
@@ -284,10 +285,10 @@ __global__ void __launch_bounds__(256) k_dmma_probe(int iters, double a, double 
 // launchers
 // ---------------------------------------------------------------------------------------------------------------------
 void launch_tables(const FpDev &d, const double *omega, const double *eig, const double *vg, const double *masses_dev,
-                   double hbar_over_kb, ModeRec *rec, float4 *recf, float2 *recn, double *occ, double2 *evec, double2 *evecc, double2 *ph1d, int *qc,
+                   double hbar_over_kb, ModeRec *rec, float4 *recf, float2 *recn, double *occ, double2 *aux, double2 *evec, double2 *evecc, double2 *ph1d, int *qc,
                    float2 *qmm, unsigned long long *maxima, cudaStream_t st) {
     cudaMemsetAsync(maxima, 0, 2 * sizeof(unsigned long long), st);
-    k_tables<<<592, 256, 0, st>>>(d, omega, eig, vg, masses_dev, hbar_over_kb, rec, recf, recn, occ, evec, evecc, ph1d, qc, qmm, maxima);
+    k_tables<<<592, 256, 0, st>>>(d, omega, eig, vg, masses_dev, hbar_over_kb, rec, recf, recn, occ, aux, evec, evecc, ph1d, qc, qmm, maxima);
 }
 
 void launch_count(int order, const FpDev &d, const RowArgs &ra, int64_t nrows, uint32_t *counts, cudaStream_t st) {

@@ -21,9 +21,7 @@
 //   V = sum_b phi(s2 qx, dR_b) sum_{xy} Mhat_b[x][y] A(atomA_b,x) conj(e~_B(atomB_b,y)),
 // where the blocks b=(atomA,atomB,dR) merge all clusters that differ only in legs already fixed by the row, and
 // Mhat_b folds the IFC values with the fixed legs' eigenvectors and phases.  A = e~_A (s2=+) or conj(e~_A) (s2=-).
-#include <mutex>
-
-#include "fp_device.cuh"
+#include "fp_contract.cuh"
 
 namespace {
 
@@ -74,144 +72,6 @@ __global__ void __launch_bounds__(256) k_pre4(FpDev d, IfcDev f, const int32_t *
             s.x = fma(v, e.x, s.x); s.y = fma(v, e.y, s.y);
         }
         t0[(size_t)t * f.n * 27 + o] = cmul(s, ph);
-    }
-}
-
-// ---------------------------------------------------------------------------------------------------------------------
-// a5 / a6 / a7: contraction + weights
-// ---------------------------------------------------------------------------------------------------------------------
-struct BlkSmem {
-    double2 *M;        // nblk*9   Mhat_b[x][y]
-    int4 *meta;        // nblk     {atomA | atomB<<16, d1, d2, d3}
-    double2 *ph;       // L
-    int *seg;          // nat*nat+1
-};
-
-// One block: u = sum_y (sum_x M[x][y] A[x]) Bc[y];  V += u * phase          (13 complex MAC = 52 DFMA)
-__device__ __forceinline__ void block_term(const double2 *M, const double2 *A, const double2 *Bc, double2 ph, double2 &V) {
-    double2 u = make_double2(0.0, 0.0);
-#pragma unroll
-    for (int y = 0; y < 3; y++) {
-        double2 t = make_double2(0.0, 0.0);
-#pragma unroll
-        for (int x = 0; x < 3; x++) cfma(t, M[3 * x + y], A[x]);
-        cfma(u, t, Bc[y]);
-    }
-    cfma(V, u, ph);
-}
-
-// NAT > 0: eigenvectors of both free legs live in registers, block loop statically split by (atomA, atomB).
-// NAT == 0: generic atom count, eigenvector components are fetched per block (L1/L2-resident table).
-// eA points at e~_A (s2=+) or conj(e~_A) (s2=-), eB at conj(e~_B); bs.ph holds phi (s2=+) or conj(phi) (s2=-): the
-// conjugations of step 6 are table choices made once per row, not arithmetic in the loop.
-template <int NAT>
-__device__ __forceinline__ double2 contract_process(const FpDev &d, const BlkSmem &bs, const double2 *__restrict__ eA,
-                                                    const double2 *__restrict__ eB, const double2 *A, const double2 *Bc,
-                                                    int3 qmx) {
-    double2 V = make_double2(0.0, 0.0);
-    if constexpr (NAT > 0) {                                         // A, Bc: registers, loaded by the caller
-#pragma unroll
-        for (int a = 0; a < NAT; a++)
-#pragma unroll
-            for (int c = 0; c < NAT; c++) {
-                const int b1 = bs.seg[a * NAT + c + 1];
-                for (int b = bs.seg[a * NAT + c]; b < b1; b++) {
-                    const int4 m = bs.meta[b];
-                    block_term(bs.M + 9 * b, A + 3 * a, Bc + 3 * c, bs.ph[phase_idx(d, qmx, m.y, m.z, m.w)], V);
-                }
-            }
-    } else {
-        const int nat = d.nat;
-        for (int a = 0; a < nat; a++) {                              // blocks are sorted by (atomA, atomB): one
-            double2 Ag[3];                                           // eigenvector fetch per group, not per block
-#pragma unroll
-            for (int x = 0; x < 3; x++) Ag[x] = __ldg(eA + 3 * a + x);
-            for (int c = 0; c < nat; c++) {
-                const int b0 = bs.seg[a * nat + c], b1 = bs.seg[a * nat + c + 1];
-                if (b0 == b1) continue;
-                double2 Bg[3];
-#pragma unroll
-                for (int x = 0; x < 3; x++) Bg[x] = __ldg(eB + 3 * c + x);
-                for (int b = b0; b < b1; b++) {
-                    const int4 m = bs.meta[b];
-                    block_term(bs.M + 9 * b, Ag, Bg, bs.ph[phase_idx(d, qmx, m.y, m.z, m.w)], V);
-                }
-            }
-        }
-    }
-    return V;
-}
-
-
-// Two processes per lane against one pass over the row's blocks: every Mhat_b read from shared memory feeds 2 x 13
-// complex MACs, and the two dependency chains interleave (NAT > 0 only).
-template <int NAT>
-__device__ __forceinline__ void contract_process2(const FpDev &d, const BlkSmem &bs, const double2 *A0, const double2 *B0,
-                                                  int3 q0, const double2 *A1, const double2 *B1, int3 q1, double2 &V0,
-                                                  double2 &V1) {
-    V0 = make_double2(0.0, 0.0); V1 = make_double2(0.0, 0.0);
-#pragma unroll
-    for (int a = 0; a < NAT; a++)
-#pragma unroll
-        for (int c = 0; c < NAT; c++) {
-            const int b1 = bs.seg[a * NAT + c + 1];
-            for (int b = bs.seg[a * NAT + c]; b < b1; b++) {
-                const int4 m = bs.meta[b];
-                const double2 p0 = bs.ph[phase_idx(d, q0, m.y, m.z, m.w)], p1 = bs.ph[phase_idx(d, q1, m.y, m.z, m.w)];
-                const double2 *M = bs.M + 9 * b;
-                double2 u0 = make_double2(0.0, 0.0), u1 = make_double2(0.0, 0.0);
-#pragma unroll
-                for (int y = 0; y < 3; y++) {
-                    double2 t0 = make_double2(0.0, 0.0), t1 = make_double2(0.0, 0.0);
-#pragma unroll
-                    for (int x = 0; x < 3; x++) {
-                        const double2 mm = M[3 * x + y];
-                        cfma(t0, mm, A0[3 * a + x]); cfma(t1, mm, A1[3 * a + x]);
-                    }
-                    cfma(u0, t0, B0[3 * c + y]); cfma(u1, t1, B1[3 * c + y]);
-                }
-                cfma(V0, u0, p0); cfma(V1, u1, p1);
-            }
-        }
-}
-
-// The same for any atom count: eigenvector components are fetched per atom group (A once per atomA, B once per
-// (atomA, atomB) pair with blocks), every Mhat_b read feeds both processes.
-__device__ __forceinline__ void contract_process2_generic(const FpDev &d, const BlkSmem &bs, const double2 *__restrict__ eA0,
-                                                          const double2 *__restrict__ eB0, int3 q0,
-                                                          const double2 *__restrict__ eA1, const double2 *__restrict__ eB1,
-                                                          int3 q1, double2 &V0, double2 &V1) {
-    V0 = make_double2(0.0, 0.0); V1 = make_double2(0.0, 0.0);
-    const int nat = d.nat;
-    for (int a = 0; a < nat; a++) {
-        if (bs.seg[a * nat] == bs.seg[(a + 1) * nat]) continue;
-        double2 A0[3], A1[3];
-#pragma unroll
-        for (int x = 0; x < 3; x++) { A0[x] = __ldg(eA0 + 3 * a + x); A1[x] = __ldg(eA1 + 3 * a + x); }
-        for (int c = 0; c < nat; c++) {
-            const int b0 = bs.seg[a * nat + c], b1 = bs.seg[a * nat + c + 1];
-            if (b0 == b1) continue;
-            double2 B0[3], B1[3];
-#pragma unroll
-            for (int y = 0; y < 3; y++) { B0[y] = __ldg(eB0 + 3 * c + y); B1[y] = __ldg(eB1 + 3 * c + y); }
-            for (int b = b0; b < b1; b++) {
-                const int4 m = bs.meta[b];
-                const double2 p0 = bs.ph[phase_idx(d, q0, m.y, m.z, m.w)], p1 = bs.ph[phase_idx(d, q1, m.y, m.z, m.w)];
-                const double2 *M = bs.M + 9 * b;
-                double2 u0 = make_double2(0.0, 0.0), u1 = make_double2(0.0, 0.0);
-#pragma unroll
-                for (int y = 0; y < 3; y++) {
-                    double2 t0 = make_double2(0.0, 0.0), t1 = make_double2(0.0, 0.0);
-#pragma unroll
-                    for (int x = 0; x < 3; x++) {
-                        const double2 mm = M[3 * x + y];
-                        cfma(t0, mm, A0[x]); cfma(t1, mm, A1[x]);
-                    }
-                    cfma(u0, t0, B0[y]); cfma(u1, t1, B1[y]);
-                }
-                cfma(V0, u0, p0); cfma(V1, u1, p1);
-            }
-        }
     }
 }
 
@@ -535,184 +395,6 @@ __global__ void __launch_bounds__(RT, RATES_MINB) k_rates(FpDev d, IfcDev f, Row
     }
 }
 
-// ---------------------------------------------------------------------------------------------------------------------
-// split path (the default): process lists in HBM, Algorithm 3 -> Algorithm 4 of the paper with both
-// halves on the device.  The enumerator needs ~40 registers and no FP64 pipe, the evaluator 128 registers and little
-// else: as separate kernels each runs at its own occupancy, and (on two streams) the enumerator of the next chunk of
-// rows fills the issue slots the FP64-bound evaluator leaves empty.
-//
-// List layout: every (row, warp) owns a slot of capw entries (capw = all candidates the warp can meet, so nothing can
-// overflow; untouched slot space costs no traffic); wcnt[row*RW + warp] is the number of entries written.  Entry order
-// inside a slot is the enumerator's (deterministic), so sums are reproducible run to run.
-// ---------------------------------------------------------------------------------------------------------------------
-static_assert(RW == 4, "k_eval reads the four warp counts of a row as one uint4");
-
-// Enumerator: stage 1 and 2 of the FP32 pre-filter, then -- for the survivors only -- the pinned FP64 decision
-// (SURVEY.md §8(c) step 3), which alone determines what is written, and the row-independent part of the
-// weight (a7).  With ~48 registers per thread ten CTAs fit on an SM, which hides the gather latency of the decision.
-template <int ORDER, int TILE, bool ONE_SUB>
-__global__ void __launch_bounds__(RT, 8) k_enum(FpDev d, RowArgs ra, int64_t capw, ListEnt *lists, uint32_t *wcnt,
-                                                uint32_t *pcnt) {
-    __shared__ uint32_t pendq[RW * PCAP];
-    const int64_t r = blockIdx.x;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const Row row = make_row<ORDER>(d, ra, ra.row0 + r);
-    unsigned nout = 0, nadm = 0, nproc = 0;
-    bool ovf = false;                                                 // the slot filled up: the row is redone by k_rates
-    // pair symmetry (fp_set_symmetry): in the 3ph - and the 4ph +- and -- channels (s2 < 0) the two free legs enter V and the
-    // weight in the same way, so only mode A <= mode B is listed; its entry carries the weights of both orderings, each with its own
-    // window decision in the pinned arithmetic
-    const bool sym = ra.sym && row.s2 < 0;
-    if (row.valid && !row_is_empty(d, row)) {                         // item 8: zero modes are never a leg
-        ListEnt *out = lists + ((size_t)r * RW + warp) * (size_t)capw;
-        uint32_t *pend = pendq + warp * PCAP;
-        const float basef = (float)row.Obase;
-        const Steps<TILE, ONE_SUB> steps(d);
-        int wp = 0;
-        for (int step = warp; step < steps.nsteps; step += RW) {
-            int tile, ja0, jb0;
-            steps.decode(step, tile, ja0, jb0);
-            wp = stage1_step<TILE>(d, row, basef, tile, ja0, jb0, lane, pend, wp, sym);
-            __syncwarp();
-            const bool last = step + RW >= steps.nsteps;
-            while (wp >= 32 || (last && wp > 0)) {                    // stage 2, 32 pending candidates at a time
-                const int n = wp < 32 ? wp : 32;
-                wp -= n;
-                const bool in = lane < n;
-                const uint32_t c2 = pend[wp + (in ? lane : 0)];
-                // stage 2 and the loads of stage 3 are issued together (one L2 round trip instead of two; a quarter of the
-                // FP64 records is fetched for candidates stage 2 then rejects)
-                const int qx = (int)(c2 >> 12), ja = (int)((c2 >> 6) & 63u), jb = (int)(c2 & 63u);
-                const int ql = q_index(d, q_add(d, row.qb, row.s2, unpack_qc(__ldg(d.qc + qx))));
-                const int p = qx * d.nb + ja, lamB = ql * d.nb + jb;
-                const uint2 e2 = make_uint2(((uint32_t)qx << 6) | (uint32_t)ja, ((uint32_t)ql << 6) | (uint32_t)jb);
-                const float4 Af = __ldg(d.recf + p), Bf = __ldg(d.recf + lamB);
-                const ModeRec a = load_rec(d.rec + p), b = load_rec(d.rec + lamB);
-                const double fa = __ldg(d.occ + p), fb = __ldg(d.occ + lamB);
-                const float dl = (row.s2 > 0 ? basef + Af.x : basef - Af.x) - Bf.x;
-                const float dx = Af.y - Bf.y, dy = Af.z - Bf.z, dz = Af.w - Bf.w;
-                const bool pass = in && dl * dl <= fmaf(d.pfK1, fmaf(dz, dz, fmaf(dy, dy, dx * dx)), d.pfC2);
-                bool ok = false;
-                double w = 0.0;
-                if (pass) {                                           // stage 3: the decision, in the pinned arithmetic
-                    const double sig = sigma_pinned(d, a, b);
-                    const double delta = __dsub_rn(row.s2 > 0 ? __dadd_rn(row.Obase, a.omega) : __dsub_rn(row.Obase, a.omega), b.omega);
-                    ok = a.omega != 0.0 && b.omega != 0.0 && sig > 0.0 && fabs(delta) <= __dmul_rn(d.ncut, sig);
-                    // weight without the row factors: occ(f_A, f_B) g / (omega_A omega_B),  g = exp(-(Delta/sigma)^2)/(sigma sqrt(pi))
-                    const double W = a.omega * b.omega;
-                    const double t = 1.0 / (sig * W);
-                    const double rr = delta * (t * W);
-                    double occ;
-                    if (ORDER == 3) occ = row.s2 > 0 ? (fa - fb) : (fa + fb + 1.0);   // symmetric in (A, B) for s2 < 0
-                    else occ = (row.s2 > 0 ? 1.0 + fa : fa) * fb;
-                    w = occ * (exp(-(rr * rr)) * t * 0.56418958354775628695);   // 1/sqrt(pi)
-                    if (!ok) w = 0.0;
-                    if (sym) {                                        // the other ordering: Delta' = (Obase - omega_B) - omega_A
-                        const double delta2 = __dsub_rn(__dsub_rn(row.Obase, b.omega), a.omega);
-                        const bool ok2 = p != lamB &&                 // (A = B is its own partner: one process; only a fixed sigma admits it)
-                                         a.omega != 0.0 && b.omega != 0.0 && sig > 0.0 && fabs(delta2) <= __dmul_rn(d.ncut, sig);
-                        if (ok2) {
-                            const double r2 = delta2 * (t * W);
-                            w += delta2 == delta ? occ * (exp(-(rr * rr)) * t * 0.56418958354775628695)
-                                                 : occ * (exp(-(r2 * r2)) * t * 0.56418958354775628695);
-                        }
-                        nproc += (ok ? 1u : 0u) + (ok2 ? 1u : 0u);
-                        ok = ok || ok2;
-                    } else {
-                        nproc += ok ? 1u : 0u;
-                    }
-                }
-                const unsigned bal = __ballot_sync(0xffffffffu, ok);
-                if (nout + __popc(bal) > (unsigned)capw) ovf = true;  // warp-uniform
-                else {
-                    if (ok) {
-                        ListEnt e; e.x = e2.x; e.y = e2.y; e.w = w;
-                        out[nout + __popc(bal & ((1u << lane) - 1u))] = e;
-                    }
-                    nout += __popc(bal);
-                }
-                nadm += pass ? 1u : 0u;
-            }
-            __syncwarp();
-        }
-    }
-    for (int o = 16; o > 0; o >>= 1) nproc += __shfl_down_sync(0xffffffffu, nproc, o);
-    if (lane == 0) {
-        wcnt[r * RW + warp] = ovf ? 0xffffffffu : nout;
-        pcnt[r * RW + warp] = nproc;
-        if (ovf) atomicAdd(ra.overflow, 1u);
-        else if (ra.evaluated && nout) atomicAdd(ra.evaluated, (unsigned long long)nout);
-    }
-    if (ra.prefiltered) {                                             // profiling only: pre-filter survivors
-        for (int o = 16; o > 0; o >>= 1) nadm += __shfl_down_sync(0xffffffffu, nadm, o);
-        if (lane == 0 && nadm) atomicAdd(ra.prefiltered, (unsigned long long)nadm);
-    }
-}
-
-// Evaluator: |V|^2 of every listed process (level-2 contraction) and the row sums.  Every entry is an allowed process,
-// so the row count is the list length; the row factors of the weight (1/omega[omega'], occupation of lambda') multiply
-// the sums once.
-// k_eval: two processes per lane, 168 registers, 3 CTAs per SM
-template <int ORDER, int NAT>
-__global__ void __launch_bounds__(EVT, 3 * (RT / EVT)) k_eval(FpDev d, IfcDev f, RowArgs ra, const double2 *pre, int64_t capw,
-                                                      const ListEnt *lists, const uint32_t *wcnt, const uint32_t *pcnt,
-                                                      double2 *partial, uint32_t *counts) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ double red[32];
-    const int64_t r = blockIdx.x;
-    const uint4 wc = __ldg(reinterpret_cast<const uint4 *>(wcnt) + r);
-    const bool ovf = (wc.x & wc.y & wc.z & wc.w) == 0xffffffffu || wc.x == 0xffffffffu || wc.y == 0xffffffffu ||
-                     wc.z == 0xffffffffu || wc.w == 0xffffffffu;      // a slot of the row filled up: redone by k_rates
-    const unsigned p1 = wc.x, p2 = p1 + wc.y, p3 = p2 + wc.z, total = ovf ? 0u : p3 + wc.w;
-    if (total == 0) {                                                 // (0xffffffff marks the row for the redo pass)
-        if (threadIdx.x == 0) { partial[r] = make_double2(0.0, 0.0); counts[r] = ovf ? 0xffffffffu : 0u; }
-        return;
-    }
-    const Row row = make_row<ORDER>(d, ra, ra.row0 + r);
-    BlkSmem bs;
-    RowWeights rw;
-    setup_row_tables<ORDER>(d, f, row, pre, smem_raw, bs, rw);
-
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const ListEnt *slot = lists + (size_t)r * RW * (size_t)capw;
-    // the four slots of the row read as one list: entry i lives in slot w = #{k : i >= p_k} at offset i - p_w
-    auto fetch = [&](unsigned i) -> ListEnt {
-        const unsigned w = (i >= p1) + (i >= p2) + (i >= p3);
-        const unsigned off = i - (w == 0 ? 0u : w == 1 ? p1 : w == 2 ? p2 : p3);
-        const uint4 v = __ldg(reinterpret_cast<const uint4 *>(slot + (size_t)w * (size_t)capw + off));
-        ListEnt e; e.x = v.x; e.y = v.y; e.w = __hiloint2double((int)v.w, (int)v.z);
-        return e;
-    };
-    double sG = 0.0, sW = 0.0;
-    for (unsigned base = warp * 64; base < total; base += 2 * EVT) {   // 64 processes per warp pass, two per lane
-        const bool act0 = base + lane < total, act1 = base + 32 + lane < total;
-        const ListEnt e0 = fetch(act0 ? base + lane : base), e1 = fetch(act1 ? base + 32 + lane : base);
-        const int qx0 = (int)(e0.x >> 6), qx1 = (int)(e1.x >> 6);
-        const double2 *eA0 = (row.s2 > 0 ? d.evec : d.evecc) + ((size_t)qx0 * d.nb + (e0.x & 63u)) * d.nb;
-        const double2 *eA1 = (row.s2 > 0 ? d.evec : d.evecc) + ((size_t)qx1 * d.nb + (e1.x & 63u)) * d.nb;
-        const double2 *eB0 = d.evecc + ((size_t)(e0.y >> 6) * d.nb + (e0.y & 63u)) * d.nb;
-        const double2 *eB1 = d.evecc + ((size_t)(e1.y >> 6) * d.nb + (e1.y & 63u)) * d.nb;
-        const int3 xc0 = unpack_qc(__ldg(d.qc + qx0)), xc1 = unpack_qc(__ldg(d.qc + qx1));
-        double2 V0, V1;
-        if constexpr (NAT > 0) {
-            double2 A0[3 * (NAT > 0 ? NAT : 1)], B0[3 * (NAT > 0 ? NAT : 1)], A1[3 * (NAT > 0 ? NAT : 1)], B1[3 * (NAT > 0 ? NAT : 1)];
-            load_evec<3 * NAT>(eA0, A0); load_evec<3 * NAT>(eB0, B0); load_evec<3 * NAT>(eA1, A1); load_evec<3 * NAT>(eB1, B1);
-            contract_process2<NAT>(d, bs, A0, B0, premul(d, xc0), A1, B1, premul(d, xc1), V0, V1);
-        } else {
-            contract_process2_generic(d, bs, eA0, eB0, premul(d, xc0), eA1, eB1, premul(d, xc1), V0, V1);
-        }
-        if (act0) { sW += e0.w; sG = fma(e0.w, V0.x * V0.x + V0.y * V0.y, sG); }
-        if (act1) { sW += e1.w; sG = fma(e1.w, V1.x * V1.x + V1.y * V1.y, sG); }
-    }
-    const double rowfac = rw.occ_row / rw.wrow;
-    const double tG = block_sum<double>(sG, red);
-    const double tW = block_sum<double>(sW, red);
-    if (threadIdx.x == 0) {                                           // processes: both orderings of a listed pair count
-        const uint4 pc = __ldg(reinterpret_cast<const uint4 *>(pcnt) + r);
-        partial[r] = make_double2(rowfac * tG, rowfac * tW); counts[r] = pc.x + pc.y + pc.z + pc.w;
-    }
-}
-
 }  // namespace
 
 // ---------------------------------------------------------------------------------------------------------------------
@@ -732,24 +414,6 @@ static size_t tables_smem_bytes(const FpDev &d, const IfcDev &f) {
 size_t rates_smem_bytes(const FpDev &d, const IfcDev &f) {
     size_t b = tables_smem_bytes(d, f) + (size_t)(RW * QCAP + RW * 32) * sizeof(uint2) + (size_t)(RW * PCAP) * sizeof(uint32_t);
     return (b + 15) & ~(size_t)15;
-}
-
-// Dynamic shared memory above 48 KB needs an opt-in per kernel AND per device (the attribute is a per-device setting):
-// the granted size is cached per (kernel instantiation, device), under a lock.
-struct SmemGrant { std::mutex mu; size_t granted[64] = {}; };
-template <typename K>
-static cudaError_t opt_in_smem(K kernel, size_t smem, SmemGrant &g) {   // opt-in limit is 227 KB minus the static part
-    if (smem <= 48 * 1024) return cudaSuccess;
-    int dev = 0;
-    cudaError_t e = cudaGetDevice(&dev);
-    if (e != cudaSuccess) return e;
-    std::lock_guard<std::mutex> lock(g.mu);
-    if (dev < 0 || dev >= 64 || smem > g.granted[dev]) {
-        e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        if (dev >= 0 && dev < 64) g.granted[dev] = smem;
-    }
-    return cudaSuccess;
 }
 
 template <int ORDER, int NAT, int TILE>
@@ -776,58 +440,5 @@ cudaError_t launch_rates(int order, const FpDev &d, const IfcDev &f, const RowAr
     if (d.nat == 1) return launch_rates_t<4, 1, 3>(FP_ARGS);
     if (d.nat == 2) return launch_rates_t<4, 2, 6>(FP_ARGS);
     return t6 ? launch_rates_t<4, 0, 6>(FP_ARGS) : launch_rates_t<4, 0, 3>(FP_ARGS);
-#undef FP_ARGS
-}
-
-// ---- split path ------------------------------------------------------------------------------------------------------
-// entries one warp of k_enum can write for one row: its share of the sub-tile steps, every candidate admitted
-int64_t enum_slot_entries(const FpDev &d) {
-    const int tile = d.nb % 6 == 0 ? 6 : 3;
-    const int64_t nsub = d.nb / tile, nsteps = (int64_t)((d.N + 31) >> 5) * nsub * nsub;
-    return (nsteps + RW - 1) / RW * 32 * tile * tile;
-}
-int enum_warps_per_row() { return RW; }
-
-cudaError_t launch_enum(int order, const FpDev &d, const RowArgs &ra, int64_t nrows, int64_t capw, ListEnt *lists,
-                        uint32_t *wcnt, uint32_t *pcnt, cudaStream_t st) {
-    if (nrows <= 0) return cudaSuccess;
-    const unsigned g = (unsigned)nrows;
-#define FP_ENUM(O, T, S) k_enum<O, T, S><<<g, RT, 0, st>>>(d, ra, capw, lists, wcnt, pcnt)
-    if (order == 3) {
-        if (d.nb == 6) FP_ENUM(3, 6, true); else if (d.nb == 3) FP_ENUM(3, 3, true);
-        else if (d.nb % 6 == 0) FP_ENUM(3, 6, false); else FP_ENUM(3, 3, false);
-    } else {
-        if (d.nb == 6) FP_ENUM(4, 6, true); else if (d.nb == 3) FP_ENUM(4, 3, true);
-        else if (d.nb % 6 == 0) FP_ENUM(4, 6, false); else FP_ENUM(4, 3, false);
-    }
-#undef FP_ENUM
-    return cudaGetLastError();
-}
-
-template <int ORDER, int NAT>
-static cudaError_t launch_eval_t(const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const double2 *pre,
-                                 int64_t capw, const ListEnt *lists, const uint32_t *wcnt, const uint32_t *pcnt,
-                                 double2 *partial, uint32_t *counts, cudaStream_t st) {
-    const size_t smem = (tables_smem_bytes(d, f) + 15) & ~(size_t)15;
-    static SmemGrant granted;
-    cudaError_t e = opt_in_smem(k_eval<ORDER, NAT>, smem, granted);
-    if (e != cudaSuccess) return e;
-    k_eval<ORDER, NAT><<<(unsigned)nrows, EVT, smem, st>>>(d, f, ra, pre, capw, lists, wcnt, pcnt, partial, counts);
-    return cudaGetLastError();
-}
-
-cudaError_t launch_eval(int order, const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const double2 *pre,
-                        int64_t capw, const ListEnt *lists, const uint32_t *wcnt, const uint32_t *pcnt, double2 *partial,
-                        uint32_t *counts, cudaStream_t st) {
-    if (nrows <= 0) return cudaSuccess;
-#define FP_ARGS d, f, ra, nrows, pre, capw, lists, wcnt, pcnt, partial, counts, st
-    if (order == 3) {
-        if (d.nat == 1) return launch_eval_t<3, 1>(FP_ARGS);
-        if (d.nat == 2) return launch_eval_t<3, 2>(FP_ARGS);
-        return launch_eval_t<3, 0>(FP_ARGS);
-    }
-    if (d.nat == 1) return launch_eval_t<4, 1>(FP_ARGS);
-    if (d.nat == 2) return launch_eval_t<4, 2>(FP_ARGS);
-    return launch_eval_t<4, 0>(FP_ARGS);
 #undef FP_ARGS
 }

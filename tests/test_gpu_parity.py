@@ -353,9 +353,10 @@ def test_full_size_config4_sampled(fp):
 
 
 def test_list_overflow_falls_back_to_fused(fp):
-    """With the filter disabled every candidate is allowed, so the split path's list slots (a quarter of the candidates,
-    at least 2048 entries) fill up on an 8x8x8 mesh: k_enum flags them and the driver redoes the super-chunk fused."""
-    inp = fp_inputs.make_tiny("diamond", mesh=(8, 8, 8))
+    """With the filter disabled every candidate is allowed, so the list slots of the group path (a quarter of the
+    candidates a unit can meet, at least 2048 entries) fill up on a 16x8x8 mesh (two 32-point tiles per unit: 2304
+    candidates): k_enum_g marks the rows whose slot filled up and the driver redoes those rows through the fused kernel."""
+    inp = fp_inputs.make_tiny("diamond", mesh=(16, 8, 8))
     t = np.ascontiguousarray(inp.targets4[[100, 205]])
     kw = dict(ncut=np.inf, sigma_const=5.0)
     og, ow, oc = _oracle(inp, **kw).rates4(t, 5, 6)
