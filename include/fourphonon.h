@@ -167,6 +167,13 @@ int fp_set_path(fp_ctx *ctx, int path);
 int fp_set_symmetry(fp_ctx *ctx, int on);
 int fp_get_symmetry(const fp_ctx *ctx);
 
+/* Self-check of the FP32 pre-filter (DESIGN.md §5.2 claims it admits a superset of the candidates the pinned FP64 window
+ * decision of PAPER.md:163,293 allows, so that counts and rates never depend on it).  fp_set_prefilter(ctx, 0) disables
+ * every FP32 test -- each candidate then takes the pinned FP64 decision, 10-50x slower -- and fp_set_prefilter(ctx, 1)
+ * restores the constants fp_setup derived.  Counts must be bit-identical either way (tests/test_gpu_fullsize.py).
+ * Returns FP_OK or FP_EINVAL (null ctx).                                                                              */
+int fp_set_prefilter(fp_ctx *ctx, int on);
+
 /* Profiling of the library's own kernels (off by default; adds two cudaEventRecord per launch).                     */
 int fp_profile_enable(fp_ctx *ctx, int on);
 int fp_profile_reset(fp_ctx *ctx);

@@ -441,6 +441,7 @@ int fp_setup(const fp_crystal *crystal, const double *masses, const double *omeg
         } else {                                                      // ncut = inf: every pair can hold every row
             d.gfC = 0.0f; d.gfD = INFINITY; d.gfW = INFINITY;
         }
+        d.pfOff = 0;
         d.thrC = d.ncut * d.scale / std::sqrt(6.0);
         d.invC = d.sigma_const > 0.0 ? 1.0 / d.sigma_const : std::sqrt(6.0) / d.scale;
     }
@@ -796,6 +797,25 @@ int fp_set_path(fp_ctx *ctx, int path) {
 int fp_set_symmetry(fp_ctx *ctx, int on) { if (!ctx) return FP_EINVAL; ctx->use_sym = on != 0; return FP_OK; }
 int fp_get_symmetry(const fp_ctx *ctx) {
     return ctx ? ((ctx->use_sym && ctx->sym23 ? 1 : 0) | (ctx->use_sym && ctx->sym34 ? 2 : 0)) : FP_EINVAL;
+}
+
+int fp_set_prefilter(fp_ctx *ctx, int on) {
+    if (!ctx) return FP_EINVAL;
+    FpDev &d = ctx->d;
+    if (!on && !ctx->pf_saved) {                                      // every FP32 test admits everything that is not a zero mode
+        ctx->sv_pfK1 = d.pfK1; ctx->sv_pfC2 = d.pfC2; ctx->sv_pfNmax = d.pfNmax; ctx->sv_pfW = d.pfW;
+        ctx->sv_gfC = d.gfC; ctx->sv_gfD = d.gfD; ctx->sv_gfW = d.gfW;
+        d.pfK1 = 0.0f; d.pfC2 = INFINITY; d.pfNmax = INFINITY; d.pfW = INFINITY;
+        d.gfC = 0.0f; d.gfD = INFINITY; d.gfW = INFINITY;
+        d.pfOff = 1;
+        ctx->pf_saved = true;
+    } else if (on && ctx->pf_saved) {
+        d.pfK1 = ctx->sv_pfK1; d.pfC2 = ctx->sv_pfC2; d.pfNmax = ctx->sv_pfNmax; d.pfW = ctx->sv_pfW;
+        d.gfC = ctx->sv_gfC; d.gfD = ctx->sv_gfD; d.gfW = ctx->sv_gfW;
+        d.pfOff = 0;
+        ctx->pf_saved = false;
+    }
+    return FP_OK;
 }
 
 int fp_profile_enable(fp_ctx *ctx, int on) { if (!ctx) return FP_EINVAL; ctx->profiling = on != 0; return FP_OK; }

@@ -47,6 +47,7 @@ struct FpDev {
     float gfC, gfD;               // window half-width bound of a pair: bnd = gfC * |u_a - u_b|_f + gfD
     float gfW;                    // upper bound of bnd over all pairs (tile vote)
     double thrC, invC;            // ncut*scale/sqrt(6) and sqrt(6)/scale: fast path of the decision and 1/sigma
+    int pfOff;                    // fp_set_prefilter(ctx, 0): the stage-1 table of the fused kernel reads as n' = inf
 };
 
 // Anharmonic list in device layout: clusters sorted by contraction block.
@@ -109,6 +110,8 @@ struct fp_ctx {
     int path = FP_PATH_AUTO;      // fp_set_path
     bool sym34 = false, sym23 = false;   // IFC4 / IFC3 is symmetric under the exchange of its last two legs (fp_setup)
     bool use_sym = true;          // fp_set_symmetry
+    bool pf_saved = false;        // fp_set_prefilter(ctx, 0) is in effect; the constants of fp_setup are kept here:
+    float sv_pfK1 = 0, sv_pfC2 = 0, sv_pfNmax = 0, sv_pfW = 0, sv_gfC = 0, sv_gfD = 0, sv_gfW = 0;
     cudaStream_t side = nullptr;  // second stream of the split path: the enumerator of chunk k+1 runs beside the
     cudaEvent_t ev_enum[2] = {nullptr, nullptr}, ev_eval[2] = {nullptr, nullptr};   // evaluator of chunk k
     std::vector<EventRec> events;

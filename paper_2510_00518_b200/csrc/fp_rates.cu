@@ -241,14 +241,16 @@ __device__ __forceinline__ int stage1_step(const FpDev &d, const Row &row, float
     float lo[TILE], hi[TILE];
 #pragma unroll
     for (int i = 0; i < TILE; i++) {
-        const float2 A = __ldg(pa + (size_t)i * d.N);                 // omega_f = NaN for zero modes: never admitted
+        float2 A = __ldg(pa + (size_t)i * d.N);                       // omega_f = NaN for zero modes: never admitted
+        if (d.pfOff) A.y = __int_as_float(0x7f800000);               // fp_set_prefilter(ctx, 0): n' = inf
         const float ba = inq ? (row.s2 > 0 ? basef + A.x : basef - A.x) : fnan;
         lo[i] = ba - A.y; hi[i] = ba + A.y;
     }
     uint64_t mask = 0;
 #pragma unroll
     for (int k = 0; k < TILE; k++) {
-        const float2 B = __ldg(pb + (size_t)k * d.N);
+        float2 B = __ldg(pb + (size_t)k * d.N);
+        if (d.pfOff) B.y = __int_as_float(0x7f800000);
         const float bl = B.x - B.y, bh = B.x + B.y;
 #pragma unroll
         for (int i = 0; i < TILE; i++)
