@@ -148,30 +148,41 @@ __device__ __forceinline__ void contract_process2(const FpDev &d, const BlkSmem 
         }
 }
 
-// The same for any atom count: eigenvector components are fetched per atom group (A once per atomA, B once per
-// (atomA, atomB) pair with blocks), every Mhat_b read feeds both processes.
-__device__ __forceinline__ void contract_process2_generic(const FpDev &d, const BlkSmem &bs, const double2 *__restrict__ eA0,
-                                                          const double2 *__restrict__ eB0, int3 q0,
-                                                          const double2 *__restrict__ eA1, const double2 *__restrict__ eB1,
-                                                          int3 q1, double2 &V0, double2 &V1) {
+// The same for any atom count, every eigenvector component fetched once: the leg-A vectors of the two processes are
+// staged by the caller in shared memory (As[comp * 64 + 32 h], already offset by the lane: each lane reads back only
+// what it wrote), the loop runs atom-B-major with the three conj(e~_B) components of atom c in registers (those of
+// atom c + 1 are fetched while c is computed), and the sum over y is taken once per atom c:
+//   W_c[y] = sum_{b : atomB_b = c} phi_b sum_x Mhat_b[x][y] A(atomA_b, x),   V = sum_c sum_y W_c[y] conj(e~_B(c, y))
+// -- 12 complex MACs per block and process plus 3 per atom c.  Blocks are sorted by (atomA, atomB): seg[a nat + c].
+__device__ __forceinline__ void contract_process2_staged(const FpDev &d, const BlkSmem &bs, const double2 *As,
+                                                         const double2 *__restrict__ eB0, int3 q0,
+                                                         const double2 *__restrict__ eB1, int3 q1, double2 &V0, double2 &V1) {
     V0 = make_double2(0.0, 0.0); V1 = make_double2(0.0, 0.0);
     const int nat = d.nat;
-    for (int a = 0; a < nat; a++) {
-        if (bs.seg[a * nat] == bs.seg[(a + 1) * nat]) continue;
-        double2 A0[3], A1[3];
+    double2 Bn0[3], Bn1[3];
 #pragma unroll
-        for (int x = 0; x < 3; x++) { A0[x] = __ldg(eA0 + 3 * a + x); A1[x] = __ldg(eA1 + 3 * a + x); }
-        for (int c = 0; c < nat; c++) {
+    for (int y = 0; y < 3; y++) { Bn0[y] = __ldg(eB0 + y); Bn1[y] = __ldg(eB1 + y); }
+    for (int c = 0; c < nat; c++) {
+        double2 B0[3], B1[3], W0[3], W1[3];
+#pragma unroll
+        for (int y = 0; y < 3; y++) {
+            B0[y] = Bn0[y]; B1[y] = Bn1[y];
+            W0[y] = make_double2(0.0, 0.0); W1[y] = make_double2(0.0, 0.0);
+        }
+        if (c + 1 < nat) {
+#pragma unroll
+            for (int y = 0; y < 3; y++) { Bn0[y] = __ldg(eB0 + 3 * (c + 1) + y); Bn1[y] = __ldg(eB1 + 3 * (c + 1) + y); }
+        }
+        for (int a = 0; a < nat; a++) {
             const int b0 = bs.seg[a * nat + c], b1 = bs.seg[a * nat + c + 1];
             if (b0 == b1) continue;
-            double2 B0[3], B1[3];
+            double2 A0[3], A1[3];
 #pragma unroll
-            for (int y = 0; y < 3; y++) { B0[y] = __ldg(eB0 + 3 * c + y); B1[y] = __ldg(eB1 + 3 * c + y); }
+            for (int x = 0; x < 3; x++) { A0[x] = As[(3 * a + x) * 64]; A1[x] = As[(3 * a + x) * 64 + 32]; }
             for (int b = b0; b < b1; b++) {
                 const int4 m = bs.meta[b];
                 const double2 p0 = bs.ph[phase_idx(d, q0, m.y, m.z, m.w)], p1 = bs.ph[phase_idx(d, q1, m.y, m.z, m.w)];
                 const double2 *M = bs.M + 9 * b;
-                double2 u0 = make_double2(0.0, 0.0), u1 = make_double2(0.0, 0.0);
 #pragma unroll
                 for (int y = 0; y < 3; y++) {
                     double2 t0 = make_double2(0.0, 0.0), t1 = make_double2(0.0, 0.0);
@@ -180,11 +191,12 @@ __device__ __forceinline__ void contract_process2_generic(const FpDev &d, const 
                         const double2 mm = M[3 * x + y];
                         cfma(t0, mm, A0[x]); cfma(t1, mm, A1[x]);
                     }
-                    cfma(u0, t0, B0[y]); cfma(u1, t1, B1[y]);
+                    cfma(W0[y], t0, p0); cfma(W1[y], t1, p1);
                 }
-                cfma(V0, u0, p0); cfma(V1, u1, p1);
             }
         }
+#pragma unroll
+        for (int y = 0; y < 3; y++) { cfma(V0, W0[y], B0[y]); cfma(V1, W1[y], B1[y]); }
     }
 }
 

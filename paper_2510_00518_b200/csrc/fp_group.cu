@@ -404,11 +404,14 @@ struct EvalSmem {
     double *rowfac;    // ge             row factors of the weight: occ_row / (omega [omega'])
     long long *rold;   // ge             index of the row in partial[] / counts[]
     int *chunk0;       // ge + 1         first 64-process chunk of each row
-    double *accG, *accW;   // GW * ge    per (warp, row) sums
-    unsigned *accC;    // GW * ge        processes (both orderings of a listed pair count)
+    double *accG, *accW;   // nw * ge    per (warp, row) sums
+    unsigned *accC;    // nw * ge        processes (both orderings of a listed pair count)
     unsigned char *rot;  // ge           rotation of the row's chunk deal (a property of the row alone)
+    double2 *As;       // nw * nb * 64   generic atom count: leg-A eigenvectors of a warp's chunk, [component][process]
 };
-__host__ __device__ inline size_t eval_smem_layout(int ge, int nblk, int L, int nb, int nat, int NU, EvalSmem *es, unsigned char *base) {
+// nw = warps of the CTA; stage: the generic evaluator (NAT = 0) stages one eigenvector per process of every warp's chunk
+__host__ __device__ inline size_t eval_smem_layout(int ge, int nblk, int L, int nb, int nat, int NU, int nw, bool stage, EvalSmem *es,
+                                                   unsigned char *base) {
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t r = o; o += (bytes + 15) & ~(size_t)15; return r; };
     const size_t oM = take((size_t)ge * nblk * 9 * sizeof(double2)), oph = take((size_t)L * sizeof(double2)),
@@ -416,9 +419,9 @@ __host__ __device__ inline size_t eval_smem_layout(int ge, int nblk, int L, int 
                  onpk = take((size_t)nblk * sizeof(unsigned)),
                  oseg = take((size_t)(nat * nat + 1) * sizeof(int)), orowp = take((size_t)ge * (NU + 1) * sizeof(unsigned)),
                  orf = take((size_t)ge * sizeof(double)), oro = take((size_t)ge * sizeof(long long)),
-                 och = take((size_t)(ge + 1) * sizeof(int)), oaG = take((size_t)GW * ge * sizeof(double)),
-                 oaW = take((size_t)GW * ge * sizeof(double)), oaC = take((size_t)GW * ge * sizeof(unsigned)),
-                 orot = take((size_t)ge);
+                 och = take((size_t)(ge + 1) * sizeof(int)), oaG = take((size_t)nw * ge * sizeof(double)),
+                 oaW = take((size_t)nw * ge * sizeof(double)), oaC = take((size_t)nw * ge * sizeof(unsigned)),
+                 orot = take((size_t)ge), oAs = take(stage ? (size_t)nw * nb * 64 * sizeof(double2) : 0);
     if (es) {
         es->M = reinterpret_cast<double2 *>(base + oM); es->ph = reinterpret_cast<double2 *>(base + oph);
         es->e1 = reinterpret_cast<double2 *>(base + oe1); es->meta = reinterpret_cast<int4 *>(base + ometa);
@@ -426,7 +429,7 @@ __host__ __device__ inline size_t eval_smem_layout(int ge, int nblk, int L, int 
         es->rowfac = reinterpret_cast<double *>(base + orf); es->rold = reinterpret_cast<long long *>(base + oro);
         es->chunk0 = reinterpret_cast<int *>(base + och); es->accG = reinterpret_cast<double *>(base + oaG);
         es->accW = reinterpret_cast<double *>(base + oaW); es->accC = reinterpret_cast<unsigned *>(base + oaC);
-        es->rot = base + orot;
+        es->rot = base + orot; es->As = reinterpret_cast<double2 *>(base + oAs);
     }
     return o;
 }
@@ -434,14 +437,16 @@ __host__ __device__ inline size_t eval_smem_layout(int ge, int nblk, int L, int 
 #ifndef FP_EVAL_MINB
 #define FP_EVAL_MINB 3
 #endif
+constexpr int GEN_WMAX = 8;                   // warps of a generic-evaluator CTA, at most (as many as the staging leaves room for)
 template <int ORDER, int NAT, bool PH8>
-__global__ void __launch_bounds__(GT, FP_EVAL_MINB) k_eval_g(FpDev d, IfcDev f, GroupArgs ga, const double2 *pre, int64_t capw,
+__global__ void __launch_bounds__(NAT > 0 ? GT : GEN_WMAX * 32, NAT > 0 ? FP_EVAL_MINB : 1) k_eval_g(FpDev d, IfcDev f, GroupArgs ga, const double2 *pre, int64_t capw,
                                                   const ListEnt *lists, const uint32_t *wcnt, int ge, int tiles_per_group,
                                                   double2 *partial, uint32_t *counts) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ int s_nitems;
     EvalSmem es;
-    eval_smem_layout(ge, f.nblk, d.L, d.nb, d.nat, ga.nu, &es, smem_raw);
+    const int nthr = NAT > 0 ? GT : (int)blockDim.x, nw = nthr >> 5;  // (the generic evaluator picks its CTA size at launch)
+    eval_smem_layout(ge, f.nblk, d.L, d.nb, d.nat, ga.nu, nw, NAT == 0, &es, smem_raw);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nb = d.nb;
     const int NU = ga.nu;
     const int64_t gl = blockIdx.x / tiles_per_group;
@@ -451,7 +456,7 @@ __global__ void __launch_bounds__(GT, FP_EVAL_MINB) k_eval_g(FpDev d, IfcDev f, 
     if (nrt <= 0) return;
 
     // ---- the rows of the tile: list lengths, row factors ----------------------------------------------------------------
-    for (int rt = threadIdx.x; rt < nrt; rt += GT) {
+    for (int rt = threadIdx.x; rt < nrt; rt += nthr) {
         int t, lam1; int64_t rold;
         group_row<ORDER>(d, ga, G, rr0 + rt, t, lam1, rold);
         bool ovf = false;
@@ -465,7 +470,7 @@ __global__ void __launch_bounds__(GT, FP_EVAL_MINB) k_eval_g(FpDev d, IfcDev f, 
         }
         if (ovf) { total = 0; es.rpre[rt * (NU + 1) + NU] = 0; }
         es.rold[rt] = rold;
-        es.rot[rt] = (unsigned char)((ORDER == 3 ? ga.targets[t] : ga.targets[t] + lam1) & (GW - 1));
+        es.rot[rt] = (unsigned char)((unsigned)(ORDER == 3 ? ga.targets[t] : ga.targets[t] + lam1) % (unsigned)nw);
         const int lam = ga.targets[t];
         double fac = 0.0;
         if (total > 0) {
@@ -495,28 +500,28 @@ __global__ void __launch_bounds__(GT, FP_EVAL_MINB) k_eval_g(FpDev d, IfcDev f, 
 
     // ---- tables of the tile: block metadata, level 1 for every row with a list ---------------------------------------------
     const int nm9 = f.nblk * 9;
-    for (int i = threadIdx.x; i < f.nblk; i += GT) {
+    for (int i = threadIdx.x; i < f.nblk; i += nthr) {
         const int4 m = f.blk_meta[i];
         es.meta[i] = m;
         es.npk[i] = (unsigned)m.y | ((unsigned)m.z << 8) | ((unsigned)m.w << 16);
     }
-    for (int i = threadIdx.x; i <= d.nat * d.nat; i += GT) es.seg[i] = f.seg[i];
+    for (int i = threadIdx.x; i <= d.nat * d.nat; i += nthr) es.seg[i] = f.seg[i];
     if (ORDER == 3) {
         for (int rt = 0; rt < nrt; rt++) {
             if (es.rpre[rt * (NU + 1) + NU] == 0) continue;
             int t, lam1; int64_t rold;
             group_row<ORDER>(d, ga, G, rr0 + rt, t, lam1, rold);
             const double2 *src = pre + (size_t)t * nm9;
-            for (int i = threadIdx.x; i < nm9; i += GT) es.M[rt * nm9 + i] = src[i];
+            for (int i = threadIdx.x; i < nm9; i += nthr) es.M[rt * nm9 + i] = src[i];
         }
     } else {
         // level 1: Mhat_b[x][y] = sum_{c in b} phi(s1 q', Rj-Rl) sum_be T0[c][be][x][y] A'(j_c, be), A' = e~ (s1=+) or conj
-        for (int i = threadIdx.x; i < d.L; i += GT) {
+        for (int i = threadIdx.x; i < d.L; i += nthr) {
             double2 p = d.ph1d[i];
             if (G.s1 < 0) p.y = -p.y;
             es.ph[i] = p;
         }
-        for (int i = threadIdx.x; i < nrt * nb; i += GT) {
+        for (int i = threadIdx.x; i < nrt * nb; i += nthr) {
             const int rt = i / nb, c = i - rt * nb;
             const int j1 = G.j0 + (rr0 + rt) % G.nj;
             es.e1[i] = (G.s1 > 0 ? d.evec : d.evecc)[((size_t)G.q1 * nb + j1) * nb + c];
@@ -527,7 +532,7 @@ __global__ void __launch_bounds__(GT, FP_EVAL_MINB) k_eval_g(FpDev d, IfcDev f, 
         // over that member's rows (at most nb)
         const int nj = G.nj;
         const int m_lo = rr0 / nj, m_hi = (rr0 + nrt - 1) / nj;
-        for (int o = threadIdx.x; o < (m_hi - m_lo + 1) * nm9; o += GT) {
+        for (int o = threadIdx.x; o < (m_hi - m_lo + 1) * nm9; o += nthr) {
             const int mi = o / nm9, bo = o - mi * nm9;
             const int b = bo / 9, xy = bo - 9 * b;
             const int m = m_lo + mi;
@@ -560,7 +565,7 @@ __global__ void __launch_bounds__(GT, FP_EVAL_MINB) k_eval_g(FpDev d, IfcDev f, 
         }
         __syncthreads();
     }
-    for (int i = threadIdx.x; i < d.L; i += GT) {                     // phases of the free legs: phi(s2 qx, dR)
+    for (int i = threadIdx.x; i < d.L; i += nthr) {                     // phases of the free legs: phi(s2 qx, dR)
         double2 p = d.ph1d[i];
         if (G.s2 < 0) p.y = -p.y;
         es.ph[i] = p;
@@ -590,8 +595,8 @@ __global__ void __launch_bounds__(GT, FP_EVAL_MINB) k_eval_g(FpDev d, IfcDev f, 
         };
         double sG = 0.0, sW = 0.0;
         unsigned sC = 0;
-        const unsigned first = (unsigned)((warp - (int)es.rot[rt]) & (GW - 1));
-        for (unsigned base = first * 64; base < total; base += 64 * GW) {
+        const unsigned first = (unsigned)(warp - (int)es.rot[rt] + nw) % (unsigned)nw;
+        for (unsigned base = first * 64; base < total; base += 64 * nw) {
             const bool act0 = base + lane < total, act1 = base + 32 + lane < total;
             const ListEnt e0 = fetch(act0 ? base + lane : base), e1 = fetch(act1 ? base + 32 + lane : base);
             const int qx0 = (int)((e0.x & 0x7fffffffu) >> 6), qx1 = (int)((e1.x & 0x7fffffffu) >> 6);
@@ -606,7 +611,17 @@ __global__ void __launch_bounds__(GT, FP_EVAL_MINB) k_eval_g(FpDev d, IfcDev f, 
                 load_evec<3 * NAT>(eA0, A0); load_evec<3 * NAT>(eB0, B0); load_evec<3 * NAT>(eA1, A1); load_evec<3 * NAT>(eB1, B1);
                 contract_process2<NAT, PH8>(d, bs, A0, B0, premul(d, xc0), A1, B1, premul(d, xc1), V0, V1);
             } else {
-                contract_process2_generic(d, bs, eA0, eB0, premul(d, xc0), eA1, eB1, premul(d, xc1), V0, V1);
+                double2 *As = es.As + (size_t)warp * nb * 64 + lane;   // this lane's two leg-A vectors, [component][process]
+                if ((nb & 1) == 0) {
+                    for (int c = 0; c < nb; c += 2) {
+                        double2 lo, hi;
+                        ldg256(eA0 + c, lo, hi); As[c * 64] = lo; As[(c + 1) * 64] = hi;
+                        ldg256(eA1 + c, lo, hi); As[c * 64 + 32] = lo; As[(c + 1) * 64 + 32] = hi;
+                    }
+                } else {
+                    for (int c = 0; c < nb; c++) { As[c * 64] = __ldg(eA0 + c); As[c * 64 + 32] = __ldg(eA1 + c); }
+                }
+                contract_process2_staged(d, bs, As, eB0, premul(d, xc0), eB1, premul(d, xc1), V0, V1);
             }
             if (act0) { sW += e0.w; sG = fma(e0.w, V0.x * V0.x + V0.y * V0.y, sG); sC += 1u + (e0.x >> 31); }
             if (act1) { sW += e1.w; sG = fma(e1.w, V1.x * V1.x + V1.y * V1.y, sG); sC += 1u + (e1.x >> 31); }
@@ -618,11 +633,11 @@ __global__ void __launch_bounds__(GT, FP_EVAL_MINB) k_eval_g(FpDev d, IfcDev f, 
         if (lane == 0) { es.accG[warp * ge + rt] = sG; es.accW[warp * ge + rt] = sW; es.accC[warp * ge + rt] = sC; }
     }
     __syncthreads();
-    for (int r = threadIdx.x; r < nrt; r += GT) {
+    for (int r = threadIdx.x; r < nrt; r += nthr) {
         if (es.rpre[r * (NU + 1) + NU] == 0) continue;
         double tG = 0.0, tW = 0.0;
         unsigned tC = 0;
-        for (int w = 0; w < GW; w++) { tG += es.accG[w * ge + r]; tW += es.accW[w * ge + r]; tC += es.accC[w * ge + r]; }
+        for (int w = 0; w < nw; w++) { tG += es.accG[w * ge + r]; tW += es.accW[w * ge + r]; tC += es.accC[w * ge + r]; }
         const double fac = es.rowfac[r];
         partial[es.rold[r]] = make_double2(fac * tG, fac * tW);
         counts[es.rold[r]] = tC;
@@ -646,10 +661,6 @@ int64_t enum_slot_entries(const FpDev &d) {
     return (ntiles + nu - 1) / nu * 32 * d.nb * d.nb;
 }
 
-size_t eval_smem_bytes(const FpDev &d, const IfcDev &f, int ge) {
-    return eval_smem_layout(ge, f.nblk, d.L, d.nb, d.nat, enum_units(d), nullptr, nullptr);
-}
-
 cudaError_t launch_enum_g(int order, const FpDev &d, const GroupArgs &ga, int64_t ngc, int64_t capw, ListEnt *lists,
                           uint32_t *wcnt, unsigned int *work, int sm_count, cudaStream_t st) {
     if (ngc <= 0) return cudaSuccess;
@@ -665,26 +676,29 @@ cudaError_t launch_enum_g(int order, const FpDev &d, const GroupArgs &ga, int64_
     return cudaGetLastError();
 }
 
+// warps of an evaluator CTA: 4, or -- generic atom count -- as many (at most GEN_WMAX) as the per-warp staging of 64
+// leg-A eigenvectors leaves room for beside the tile's tables
+static int eval_warps(const FpDev &d, const IfcDev &f, int ge) {
+    if (d.nat <= 2) return GW;
+    int nw = GEN_WMAX;
+    while (nw > 1 && eval_smem_layout(ge, f.nblk, d.L, d.nb, d.nat, enum_units(d), nw, true, nullptr, nullptr) > 226 * 1024) nw--;
+    return nw;
+}
+size_t eval_smem_bytes(const FpDev &d, const IfcDev &f, int ge) {
+    return eval_smem_layout(ge, f.nblk, d.L, d.nb, d.nat, enum_units(d), eval_warps(d, f, ge), d.nat > 2, nullptr, nullptr);
+}
+
 template <int ORDER, int NAT>
 static cudaError_t launch_eval_t(const FpDev &d, const IfcDev &f, const GroupArgs &ga, int64_t ngc, const double2 *pre,
                                  int64_t capw, const ListEnt *lists, const uint32_t *wcnt, int ge, double2 *partial,
                                  uint32_t *counts, cudaStream_t st) {
     const size_t smem = eval_smem_bytes(d, f, ge);
     const int tiles = (ga.rmaxg + ge - 1) / ge;
-#ifndef FP_NO_PH8
-#define FP_NO_PH8 1
-#endif
-    if (NAT > 0 && d.L <= 256 && !FP_NO_PH8) {                        // phase index by dp4a
-        static SmemGrant granted;
-        cudaError_t e = opt_in_smem(k_eval_g<ORDER, NAT, (NAT > 0)>, smem, granted);
-        if (e != cudaSuccess) return e;
-        k_eval_g<ORDER, NAT, (NAT > 0)><<<(unsigned)(ngc * tiles), GT, smem, st>>>(d, f, ga, pre, capw, lists, wcnt, ge, tiles, partial, counts);
-    } else {
-        static SmemGrant granted;
-        cudaError_t e = opt_in_smem(k_eval_g<ORDER, NAT, false>, smem, granted);
-        if (e != cudaSuccess) return e;
-        k_eval_g<ORDER, NAT, false><<<(unsigned)(ngc * tiles), GT, smem, st>>>(d, f, ga, pre, capw, lists, wcnt, ge, tiles, partial, counts);
-    }
+    const unsigned nthr = 32u * (unsigned)eval_warps(d, f, ge);
+    static SmemGrant granted;
+    cudaError_t e = opt_in_smem(k_eval_g<ORDER, NAT, false>, smem, granted);
+    if (e != cudaSuccess) return e;
+    k_eval_g<ORDER, NAT, false><<<(unsigned)(ngc * tiles), nthr, smem, st>>>(d, f, ga, pre, capw, lists, wcnt, ge, tiles, partial, counts);
     return cudaGetLastError();
 }
 

@@ -351,6 +351,20 @@ int fp_setup(const fp_crystal *crystal, const double *masses, const double *omeg
         fail(ctx, FP_ENOMEM, "workspace too small for the mode tables"); return bail(FP_ENOMEM);
     }
     d.rec = rec; d.recf = recf; d.recn = recn; d.occ = occ; d.aux = aux; d.evec = evec; d.evecc = evecc; d.ph1d = ph1d; d.qc = qc; d.qmm = qmm;
+    // executed FP64 flops per matrix element: 13 complex MACs per block (nat <= 2: contract_process2); generic
+    // atom count (contract_process2_staged): 12 per block + 3 per atom B that has blocks; 8 flop per complex MAC
+    auto flops_elem = [&](const IfcHost &h) {
+        if (nat <= 2) return 8.0 * 13.0 * h.nblk;
+        int nc = 0;
+        for (int c = 0; c < nat; c++) {
+            bool any = false;
+            for (int a = 0; a < nat; a++) any = any || h.seg[a * nat + c + 1] > h.seg[a * nat + c];
+            nc += any ? 1 : 0;
+        }
+        return 8.0 * (12.0 * h.nblk + 3.0 * nc);
+    };
+    if (ifc3) ctx->flops_elem3 = flops_elem(h3);
+    if (ifc4) ctx->flops_elem4 = flops_elem(h4);
     if (ifc3) {
         int rc = upload_ifc(ctx, bump, h3, ctx->i3, st); if (rc) return bail(rc);
         ctx->has3 = true;
@@ -697,7 +711,7 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
             // are not in this figure), else one per process
             const int64_t evaluated = split ? (int64_t)hstat3[2] : total;
             ctx->prof.evaluated += evaluated;
-            ctx->prof.rates_flops += (double)evaluated * (double)f.nblk * 13.0 * 8.0;
+            ctx->prof.rates_flops += (double)evaluated * (order == 3 ? ctx->flops_elem3 : ctx->flops_elem4);
         }
     }
     return FP_OK;

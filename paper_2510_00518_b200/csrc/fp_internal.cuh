@@ -119,6 +119,7 @@ struct fp_ctx {
     fp_profile prof{};
     std::string err;
     int device = 0;               // the device fp_setup ran on
+    double flops_elem3 = 0, flops_elem4 = 0;   // executed FP64 flops per matrix element of the evaluator (profile model)
 };
 
 enum { CAT_PRE = 0, CAT_RATES, CAT_REDUCE, CAT_ENUM, CAT_N };
