@@ -25,13 +25,18 @@ ROOT = Path(__file__).resolve().parent
 if str(ROOT) not in sys.path:
     sys.path.insert(0, str(ROOT))
 
-METRIC = "4ph processes/s (FP64)"
+METRIC = "4ph processes/s (FP64)"      # (3ph-only workloads count 3ph processes; config.processes_counted_in_value says which)
 UNIT = "processes/s"
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12     # 148 SMs x 64 FP64 FMA/clk/SM x 2 flop x 1965 MHz
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the committed ncu --set full
-# captures (profiles/r1c_summary.md); keyed by (config, path).  None = not captured for that configuration.
-NCU_DRAM_BYTES_PER_LAUNCH = {(3, "split"): 1.562e9}   # k_eval<4,2>, a 43,688-row launch of config 3: 1.556 GB read (the
-#                                                        process list k_enum wrote) + 6 MB written
+NCU_TRAFFIC = ROOT / "profiles" / "ncu_traffic.json"     # dram bytes of one launch per (config, kernel), each naming its ncu capture
+
+
+def ncu_traffic(cfg: int, kernel: str):
+    """-> the tracked entry of profiles/ncu_traffic.json for this configuration's dominant kernel, or None."""
+    try:
+        return json.loads(NCU_TRAFFIC.read_text()).get(f"{cfg}:{kernel}")
+    except (OSError, ValueError):
+        return None
 
 
 def workload(cfg: int):
@@ -44,6 +49,8 @@ def workload(cfg: int):
 
 def workload_name(cfg: int) -> str:
     import fp_inputs
+    if cfg in fp_inputs.PAPER_MESHES:                                       # not a BASELINE.json config
+        return f"{fp_inputs.CONFIG_NAMES[cfg]} (fp_inputs config {cfg}; synthetic IFCs of configs 0-3)"
     return f"BASELINE.json configs[{cfg}]: {fp_inputs.CONFIG_NAMES[cfg]}"
 
 
@@ -109,7 +116,25 @@ def cpu_oracle_sample(cfg: int, budget_s: float = 15.0):
     range sized from a calibration call so that the timed call is ~budget_s of host work."""
     from oracle.oracle import Oracle
     jobs = workload(cfg)
-    inp, _, t4 = next(j for j in jobs if j[2] is not None)
+    job4 = next((j for j in jobs if j[2] is not None), None)
+    if job4 is None:                                                        # 3ph-only workloads: a sample of the target modes
+        inp, t3, _ = jobs[0]
+        orc = Oracle(inp)
+        probe = np.ascontiguousarray(t3[:: max(1, len(t3) // 8)][:8])
+        t0 = time.perf_counter()
+        orc.rates3(probe)
+        dt = max(time.perf_counter() - t0, 1e-3)
+        n = int(max(8, min(len(t3), 8 * budget_s / dt)))
+        t = np.ascontiguousarray(t3[:: max(1, len(t3) // n)][:n])
+        t0 = time.perf_counter()
+        _, _, c = orc.rates3(t)
+        dt = time.perf_counter() - t0
+        procs = int(c.sum())
+        return {"value": procs / dt, "unit": UNIT, "cores": Oracle.num_threads(), "kind": "oracle",
+                "note": "the oracle is a deliberately plain correctness checker, not a tuned CPU implementation",
+                "sample": f"oracle rates3 on {len(t)} of the {len(t3)} target modes (evenly spaced): {procs} allowed "
+                          f"processes in {dt:.2f} s"}, dt, procs
+    inp, _, t4 = job4
     orc = Oracle(inp)
     t = np.ascontiguousarray(t4[:6])
     N = inp.nq
@@ -123,6 +148,7 @@ def cpu_oracle_sample(cfg: int, budget_s: float = 15.0):
     dt = time.perf_counter() - t0
     procs = int(c.sum())
     return {"value": procs / dt, "unit": UNIT, "cores": Oracle.num_threads(), "kind": "oracle",
+            "note": "the oracle is a deliberately plain correctness checker (full rectangular domain, V from the raw IFC list per process), not a tuned CPU implementation: the GPU/CPU ratio says nothing about kernel quality",
             "sample": f"oracle rates4 on the first {len(t)} target modes, q' in [{q0},{q0 + nq}) of {N}: {procs} allowed "
                       f"processes in {dt:.2f} s"}, dt, procs
 
@@ -299,15 +325,26 @@ def main():
     probe = fp.fp_probe_fp64_tflops()
     kname = ("k_eval (V3/V4 level-2 contraction + row sums over the process lists; the enumerator k_enum is timed "
              "separately, see kernel_ms_per_step)") if split else "k_rates (fused enumerate + V3/V4 contraction + weights)"
-    traffic = NCU_DRAM_BYTES_PER_LAUNCH.get((args.config, "split" if split else "fused"))
+    tr = ncu_traffic(args.config, "k_eval_g" if split else "k_rates")
+    dmma = fp.fp_probe_dmma_tflops()
+    step_flops_rate = flops / (ms_step * 1e-3) / 1e12
     roofline = {"bound": "alu", "kernel": kname, "achieved": achieved,
-                "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS, "traffic": traffic,
-                "traffic_source": "profiles/r1f_summary.md (ncu --set full, dram bytes read + written, one launch)"
-                                  if traffic is not None else None,
+                "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS,
+                "traffic": tr["bytes"] if tr else None,
+                "traffic_source": ({"file": "profiles/ncu_traffic.json", "capture": tr["capture"], "launch": tr["launch"],
+                                    "launch_ms": tr["duration_ms"], "list_bytes_of_that_launch": tr["list_bytes"]}
+                                   if tr else None),
+                "algorithmic_bytes_per_launch_avg": 16.0 * evaluated / max(n_c, 1) if split else 20.0 * rows / max(n_c, 1),
+                "whole_step": {"achieved": step_flops_rate, "frac": step_flops_rate / FP64_PEAK_TFLOPS,
+                               "what": "the same executed-flop model over the whole device-timed step (enumerator, "
+                                       "pre-contraction and reduction included in the time, not in the flops)"},
+                "probes_tflops": {"dfma": probe, "dmma_m8n8k4": dmma["dmma"], "dfma_same_shape": dmma["dfma"],
+                                  "dmma_and_dfma_interleaved": dmma["dmma_and_dfma"]},
                 "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (MEASURED_PEAKS.json has no FP64 "
                                f"entry); DFMA probe on this GPU measured {probe:.2f} TFLOP/s",
-                "flops_model": "matrix elements evaluated x nblk x 13 complex MAC x 8 flop (DESIGN.md §6); enumeration, "
-                               "decision and weights not counted",
+                "flops_model": "matrix elements evaluated x executed flops of the level-2 contraction (nat <= 2: nblk x 13 complex "
+                               "MAC x 8 flop; generic atom count: (12 nblk + 3 atoms) x 8; DESIGN.md §6); enumeration, decision "
+                               "and weights not counted",
                 "matrix_elements_per_step": evaluated,
                 "pair_symmetry": ("on: the IFC4 list is symmetric in its last two legs, so each unordered {lambda'', lambda'''} "
                                   "pair of the +- and -- channels is evaluated once (both orderings counted as processes, "

@@ -7,5 +7,5 @@ element, no occupation factor, no rate sum.
 """
 from .generate import (  # noqa: F401
     Crystal, Inputs, diamond_crystal, sc8_crystal, sc1_crystal, spring_fc2, phonons, clusters, random_ifc,
-    make_config, make_tiny, qpoint_index, qpoint_coords, CONFIG_NAMES,
+    make_config, make_tiny, qpoint_index, qpoint_coords, CONFIG_NAMES, PAPER_MESHES,
 )

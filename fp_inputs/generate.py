@@ -33,7 +33,12 @@ CONFIG_NAMES = {
     2: "diamond 8x8x8 4ph, 32 target q x 6 branches",
     3: "diamond 16x16x16 4ph 16 target q x 6 branches + 3ph all modes + kappa",
     4: "sc8 (8 atoms, 24 branches): 3ph 12x12x12 all modes; 4ph 6x6x6 8 target q x 24 branches",
+    # the paper's own mesh sizes on the diamond crystal of configs 0-3 -- not BASELINE.json configs:
+    5: "paper mesh: diamond 32x32x32 3ph all 196,608 modes",
+    6: "paper mesh: diamond 10x10x10 3ph all modes + kappa + 4ph 32 target q x 6 branches",
+    7: "paper mesh: diamond 14x14x14 3ph all modes + kappa + 4ph 16 target q x 6 branches",
 }
+PAPER_MESHES = {5: (32, 32, 32), 6: (10, 10, 10), 7: (14, 14, 14)}
 
 
 # ------------------------------------------------------------------------------------------------------------------
@@ -394,6 +399,20 @@ def make_config(idx: int):
             else:                                  # config 3 reuses IFC3 (seed+0) and IFC4 (seed+2); its own stream
                 rng = np.random.default_rng(BASE_SEED + 3)        # draws only its 16 target q-points
                 inp.targets4 = _target_modes(rng, N, 16, 6)
+        return {"main": inp}
+    if idx in PAPER_MESHES:                        # same crystal, IFC3 (seed+0) and IFC4 (seed+2) as configs 0-3
+        cr = diamond_crystal()
+        mesh = PAPER_MESHES[idx]
+        om, eg, vg = _diamond_phonons(mesh)
+        N = int(np.prod(mesh))
+        inp = Inputs(CONFIG_NAMES[idx], cr, np.array(mesh, dtype=np.int32), om, eg, vg)
+        inp.ifc3 = _diamond_ifc3()
+        inp.targets3 = np.arange(N * 6, dtype=np.int32)
+        if idx != 5:
+            a4, c4, p4, _ = _diamond_ifc4()
+            inp.ifc4 = (a4, c4, p4)
+            rng = np.random.default_rng(BASE_SEED + idx)          # draws only the target q-points
+            inp.targets4 = _target_modes(rng, N, 32 if idx == 6 else 16, 6)
         return {"main": inp}
     if idx == 4:
         cr, fc2, i3, i4, t4 = _sc8_parts()

@@ -152,3 +152,51 @@ def test_prefilter_is_a_superset_config3_one_percent(fp):
     assert c.sum() > 10 ** 8
     c3 = _counts_filter_on_off(fp, inp, inp.targets3[::7], None, order=3)
     assert c3.sum() > 10 ** 7
+
+
+# ---- the paper's own mesh sizes: fp_inputs configs 5-7 ---------------------------
+def test_paper_mesh_32cubed_3ph_sampled(fp):
+    """3ph at 32x32x32 (196,608 modes): counts + WP of 768 targets spread over the mesh against the oracle's
+    weights-only pass, Gamma (with V) of 24 of them; the whole job runs on the bench configuration."""
+    inp = fp_inputs.make_config(5)["main"]
+    orc = _oracle(inp)
+    t = np.ascontiguousarray(inp.targets3[5::256])
+    assert len(t) == 768
+    _, ow, oc = orc.rates3(t, weights_only=True)
+    tg = np.ascontiguousarray(t[::32])
+    og, ogw, ogc = orc.rates3(tg)
+    with fp.Context.from_inputs(inp, scratch_bytes=BENCH_SCRATCH) as ctx:
+        g, w, c = ctx.rates3(t)
+        ga, wa, ca = ctx.rates3(inp.targets3)                         # all modes in one call: the same rows, bit for bit
+    assert np.array_equal(c, oc), "3ph process counts are not bit-exact at 32^3"
+    assert_rates_close(w, ow, "WP3 32^3")
+    assert np.array_equal(c[::32], ogc)
+    assert_rates_close(g[::32], og, "Gamma3 32^3")
+    assert np.array_equal(ca[5::256], c) and np.array_equal(ga[5::256], g) and np.array_equal(wa[5::256], w)
+
+
+@pytest.mark.parametrize("cfg", [6, 7])
+def test_paper_mesh_4ph_sampled_and_3ph_kappa(fp, cfg):
+    """3ph + 4ph at 10x10x10 and 14x14x14: lcm 10 / 14 is not a power of two (the `% L` phase index and
+    the table look-up of q coordinates at size).  4ph: two targets over ALL q' (counts + WP), Gamma of six branches on
+    two q'; 3ph: all modes counts + WP, kappa of the GPU's Gamma_3 against orc_kappa."""
+    inp = fp_inputs.make_config(cfg)["main"]
+    orc = _oracle(inp)
+    t2 = np.ascontiguousarray(inp.targets4[[7, 52]])
+    _counts_and_wp4(fp, inp, t2, configs=_configs(fp)[:2])
+    t6 = np.ascontiguousarray(inp.targets4[18:24])
+    q0 = inp.nq // 3
+    og, ow, oc = orc.rates4(t6, q0, q0 + 2)
+    _, ow3, oc3 = orc.rates3(inp.targets3, weights_only=True)
+    with fp.Context.from_inputs(inp, scratch_bytes=BENCH_SCRATCH) as ctx:
+        g, w, c = ctx.rates4(t6, q0, q0 + 2)
+        g3, w3, c3 = ctx.rates3(inp.targets3)
+        gt = g3.sum(axis=1)
+        k = ctx.kappa_rta(gt)
+    assert np.array_equal(c, oc)
+    assert_rates_close(g, og, f"Gamma4 config {cfg}")
+    assert_rates_close(w, ow, f"WP4 config {cfg}")
+    assert np.array_equal(c3, oc3), "3ph process counts are not bit-exact"
+    assert_rates_close(w3, ow3, f"WP3 config {cfg}")
+    ok = orc.kappa(gt)
+    assert np.abs(k - ok).max() <= RTOL * np.abs(ok).max()
