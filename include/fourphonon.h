@@ -29,6 +29,14 @@
  *   next super-chunk of targets, the bounded-memory loop of Algorithm 5), so on return the outputs
  *   are complete.  fp_kappa_rta with FP_MEM_DEVICE outputs is asynchronous.
  *
+ * Limits
+ *   natoms <= 21 (64-bit branch masks), N_mu <= 1024, N <= 2^20 q-points, lcm(N1,N2,N3) <= 4096 (phase table in shared
+ *   memory).  The clusters of an IFC list are regrouped into contraction blocks (atomA, atomB, R_A - R_B mod mesh) of
+ *   its last two legs; the per-row table of a list (144 bytes per block) lives in the shared memory of one SM, which
+ *   caps a list at about 1,400 blocks (the synthetic configs have 10-152; first-principles silicon IFC3 sets within
+ *   the usual cutoffs have a few hundred).  fp_rates3 / fp_rates4 return FP_ENOMEM beyond that and fp_last_error names
+ *   the block count.
+ *
  * Errors
  *   Every call returns FP_OK (0) or a negative code; nothing throws or aborts.  fp_last_error(ctx) (ctx may be NULL
  *   for setup failures) returns a static/ctx-owned message.
@@ -45,7 +53,7 @@ extern "C" {
 
 #define FP_OK       0
 #define FP_EINVAL  (-1)   /* bad argument / shape / value                         */
-#define FP_ENOMEM  (-2)   /* workspace too small                                  */
+#define FP_ENOMEM  (-2)   /* workspace too small, or an IFC list with too many contraction blocks (see Limits) */
 #define FP_ECUDA   (-3)   /* a CUDA runtime call or kernel failed                 */
 #define FP_ESTATE  (-4)   /* call order (e.g. fp_rates4 without IFC4 at setup)    */
 
@@ -166,6 +174,16 @@ int fp_set_path(fp_ctx *ctx, int path);
  * returns a bit mask of what is in effect: 1 = 3ph, 2 = 4ph.                                                         */
 int fp_set_symmetry(fp_ctx *ctx, int on);
 int fp_get_symmetry(const fp_ctx *ctx);
+
+/* Time-reversal reuse over targets (PAPER.md:135-136 evaluates targets of the irreducible part
+ * only).  fp_setup checks, bit for bit, that the mode arrays satisfy omega(-q,j) = omega(q,j), v(-q,j) = -v(q,j) and
+ * e(-q,j) = conj(e(q,j)).  If they do, the targets (q,j) and (-q,j) of one fp_rates3 call -- or of one fp_rates4 call over
+ * the whole q' range -- share their result: the library evaluates one of each pair present in `targets` and copies
+ * Gamma, WP and the counts to the other (the two sums run over mirrored sets of processes with bitwise equal window
+ * decisions and weights and complex-conjugate matrix elements: counts identical, rates equal to rounding order).
+ * fp_set_target_symmetry(ctx, 0) turns it off; fp_get_target_symmetry returns 1 if it is in effect.                    */
+int fp_set_target_symmetry(fp_ctx *ctx, int on);
+int fp_get_target_symmetry(const fp_ctx *ctx);
 
 /* Self-check of the FP32 pre-filter (DESIGN.md §5.2 claims it admits a superset of the candidates the pinned FP64 window
  * decision of PAPER.md:163,293 allows, so that counts and rates never depend on it).  fp_set_prefilter(ctx, 0) disables

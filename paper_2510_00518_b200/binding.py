@@ -28,7 +28,7 @@ _SOURCES = ["fp_kernels.cu", "fp_rates.cu", "fp_group.cu", "fp_host.cu"]
 # every symbol include/fourphonon.h declares (tests check that the built library exports all of them)
 EXPORTED_SYMBOLS = [
     "fp_workspace_bytes", "fp_setup", "fp_rates3", "fp_rates4", "fp_kappa_rta", "fp_list3", "fp_list4",
-    "fp_set_path", "fp_set_symmetry", "fp_get_symmetry", "fp_set_prefilter", "fp_profile_enable", "fp_profile_reset", "fp_profile_get", "fp_probe_fp64_tflops", "fp_probe_dmma_tflops", "fp_constants",
+    "fp_set_path", "fp_set_symmetry", "fp_get_symmetry", "fp_set_target_symmetry", "fp_get_target_symmetry", "fp_set_prefilter", "fp_profile_enable", "fp_profile_reset", "fp_profile_get", "fp_probe_fp64_tflops", "fp_probe_dmma_tflops", "fp_constants",
     "fp_last_error", "fp_version", "fp_destroy",
 ]
 
@@ -136,6 +136,10 @@ def load_library():
     lib.fp_set_symmetry.argtypes = [vp, C.c_int]
     lib.fp_get_symmetry.restype = C.c_int
     lib.fp_get_symmetry.argtypes = [vp]
+    lib.fp_set_target_symmetry.restype = C.c_int
+    lib.fp_set_target_symmetry.argtypes = [vp, C.c_int]
+    lib.fp_get_target_symmetry.restype = C.c_int
+    lib.fp_get_target_symmetry.argtypes = [vp]
     lib.fp_set_prefilter.restype = C.c_int
     lib.fp_set_prefilter.argtypes = [vp, C.c_int]
     lib.fp_profile_enable.restype = C.c_int
@@ -392,6 +396,14 @@ class Context:
     def set_symmetry(self, on: bool):
         """Turn the lambda'' <-> lambda''' pair reuse of the 4ph +- / -- channels on or off (include/fourphonon.h)."""
         self._check(self.lib.fp_set_symmetry(self.ctx, 1 if on else 0))
+
+    def set_target_symmetry(self, on: bool):
+        """fp_set_target_symmetry: time-reversal reuse between the targets (q,j) and (-q,j) of one call."""
+        self._check(self.lib.fp_set_target_symmetry(self.ctx, 1 if on else 0))
+
+    def get_target_symmetry(self) -> bool:
+        """True if fp_setup found the mode arrays time-reversal symmetric bit for bit and the reuse is on."""
+        return self.lib.fp_get_target_symmetry(self.ctx) > 0
 
     def set_prefilter(self, on: bool):
         """fp_set_prefilter: False disables every FP32 pre-filter test (self-check of the superset claim; slow)."""

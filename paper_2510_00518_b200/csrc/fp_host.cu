@@ -406,6 +406,36 @@ int fp_setup(const fp_crystal *crystal, const double *masses, const double *omeg
             fail(ctx, FP_EINVAL, "omega has a near-zero entry (0 < omega < 1e-6*omega_max); zero modes must be exactly 0");
             return bail(FP_EINVAL);
         }
+    {   // time-reversal check of the mode arrays (bitwise: the window decision, hence the counts, must map exactly)
+        std::vector<double> h_eig, h_vg;
+        const double *he = eig, *hv = vg;
+        if (loc != FP_MEM_HOST) {
+            h_eig.resize(M * nb * 2); h_vg.resize(M * 3);
+            CU(cudaMemcpyAsync(h_eig.data(), eig, M * nb * 16, cudaMemcpyDeviceToHost, st));
+            CU(cudaMemcpyAsync(h_vg.data(), vg, M * 24, cudaMemcpyDeviceToHost, st));
+            CU(cudaStreamSynchronize(st));
+            he = h_eig.data(); hv = h_vg.data();
+        }
+        ctx->qpartner.resize(N);
+        bool ok = true;
+        for (int i3 = 0; i3 < mesh[2]; i3++)
+            for (int i2 = 0; i2 < mesh[1]; i2++)
+                for (int i1 = 0; i1 < mesh[0]; i1++) {
+                    const size_t iq = i1 + (size_t)mesh[0] * (i2 + (size_t)mesh[1] * i3);
+                    const size_t ip = (size_t)((mesh[0] - i1) % mesh[0]) +
+                                      (size_t)mesh[0] * (((mesh[1] - i2) % mesh[1]) + (size_t)mesh[1] * ((mesh[2] - i3) % mesh[2]));
+                    ctx->qpartner[iq] = (int32_t)ip;
+                    if (!ok || ip <= iq) continue;                    // each pair once; a self-conjugate q-point needs nothing
+                    for (size_t j = 0; j < nb && ok; j++) {
+                        const size_t a = iq * nb + j, b = ip * nb + j;
+                        ok = h_omega[a] == h_omega[b] && hv[3 * a] == -hv[3 * b] && hv[3 * a + 1] == -hv[3 * b + 1] &&
+                             hv[3 * a + 2] == -hv[3 * b + 2];
+                        for (size_t c = 0; c < nb && ok; c++)
+                            ok = he[2 * (a * nb + c)] == he[2 * (b * nb + c)] && he[2 * (a * nb + c) + 1] == -he[2 * (b * nb + c) + 1];
+                    }
+                }
+        ctx->trs_ok = ok;
+    }
     CU(cudaMemcpyAsync(masses_dev, masses, nat * 8, cudaMemcpyHostToDevice, st));
     // stage 1 of the FP32 pre-filter: |Delta_f| <= n'_a + n'_b with n' = cs |u| (1+1e-6) + slack
     d.pfCs = d.sigma_const > 0.0 ? 0.5 * d.ncut * d.sigma_const : d.ncut * d.scale / std::sqrt(6.0);
@@ -488,7 +518,55 @@ int fp_destroy(fp_ctx *ctx) {
 // super-chunk of targets whose per-row partial sums fit the scratch (Algorithm 5's bounded-memory loop, PAPER.md:354-393,
 // with chunks of many modes instead of one), then the fixed-order per-mode reduction.
 static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t nt, int32_t qp_begin, int32_t qp_end,
-                        double *gamma, double *wp, int64_t *counts, fp_memloc loc, cudaStream_t st) {
+                        double *gamma, double *wp, int64_t *counts, fp_memloc loc, cudaStream_t st, bool reduce = true);
+
+// Time reversal (fp_set_target_symmetry): evaluate one target of every {(q,j), (-q,j)} pair of the list and copy its
+// rates, weighted phase space and counts to the other -- the sums of the two targets run over mirrored (q' -> -q')
+// sets of processes with bitwise equal window decisions and weights and complex-conjugate matrix elements.  Only for
+// whole q' ranges (a partial range of one target is the mirrored range of the other).
+static int rates_reduced(fp_ctx *ctx, int order, const std::vector<int32_t> &ht, int32_t qp_begin, int32_t qp_end, double *gamma,
+                         double *wp, int64_t *counts, fp_memloc loc, cudaStream_t st, bool &done) {
+    const FpDev &d = ctx->d;
+    const int64_t nt = (int64_t)ht.size();
+    const int nch = order == 3 ? 2 : 3;
+    done = false;
+    std::map<int32_t, int32_t> slot;                                  // representative mode -> index into reps
+    std::vector<int32_t> reps, where(nt);
+    for (int64_t i = 0; i < nt; i++) {
+        const int32_t q = ht[i] / d.nb, j = ht[i] - q * d.nb;
+        const int32_t r = std::min(q, ctx->qpartner[q]) * d.nb + j;
+        auto it = slot.find(r);
+        if (it == slot.end()) { it = slot.emplace(r, (int32_t)reps.size()).first; reps.push_back(r); }
+        where[i] = it->second;
+    }
+    if ((int64_t)reps.size() == nt) return FP_OK;                     // nothing to share: the caller runs the plain path
+    const size_t nr = reps.size();
+    std::vector<double> g(nr * nch), w(nr * nch), go(nt * nch), wo(nt * nch);
+    std::vector<int64_t> c(nr * nch), co(nt * nch);
+    int rc = rates_driver(ctx, order, reps.data(), (int64_t)nr, qp_begin, qp_end, g.data(), w.data(), c.data(), FP_MEM_HOST, st, false);
+    if (rc != FP_OK) return rc;
+    for (int64_t i = 0; i < nt; i++)
+        for (int k = 0; k < nch; k++) {
+            go[i * nch + k] = g[(size_t)where[i] * nch + k]; wo[i * nch + k] = w[(size_t)where[i] * nch + k];
+            co[i * nch + k] = c[(size_t)where[i] * nch + k];
+        }
+    if (ctx->profiling) {                                             // processes delivered, not only those evaluated
+        int64_t extra = 0;
+        for (int64_t v : co) extra += v;
+        for (int64_t v : c) extra -= v;
+        ctx->prof.processes += extra;
+    }
+    const cudaMemcpyKind kind = loc == FP_MEM_HOST ? cudaMemcpyHostToHost : cudaMemcpyHostToDevice;
+    CU(cudaMemcpyAsync(gamma, go.data(), go.size() * 8, kind, st));
+    if (wp) CU(cudaMemcpyAsync(wp, wo.data(), wo.size() * 8, kind, st));
+    if (counts) CU(cudaMemcpyAsync(counts, co.data(), co.size() * 8, kind, st));
+    CU(cudaStreamSynchronize(st));
+    done = true;
+    return FP_OK;
+}
+
+static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t nt, int32_t qp_begin, int32_t qp_end,
+                        double *gamma, double *wp, int64_t *counts, fp_memloc loc, cudaStream_t st, bool reduce) {
     if (!ctx) return FP_EINVAL;
     const FpDev &d = ctx->d;
     const IfcDev &f = order == 3 ? ctx->i3 : ctx->i4;
@@ -510,6 +588,11 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
     for (int64_t i = 0; i < nt; i++)
         if (ht[i] < 0 || ht[i] >= nmodes) return fail(ctx, FP_EINVAL, "target mode index out of range");
 
+    if (reduce && ctx->trs_ok && ctx->use_trs && (order == 3 || (qp_begin == 0 && qp_end == d.N))) {
+        bool done = false;
+        const int rc = rates_reduced(ctx, order, ht, qp_begin, qp_end, gamma, wp, counts, loc, st, done);
+        if (rc != FP_OK || done) return rc;
+    }
     if (nqp == 0) {                                                   // empty q' range: all outputs zero
         std::vector<double> z(nt * nch, 0.0); std::vector<int64_t> zc(nt * nch, 0);
         cudaMemcpyKind k = loc == FP_MEM_HOST ? cudaMemcpyHostToHost : cudaMemcpyHostToDevice;
@@ -519,8 +602,14 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
         CU(cudaStreamSynchronize(st));
         return FP_OK;
     }
-    if (rates_smem_bytes(d, f) > 227 * 1024 - 1024)
-        return fail(ctx, FP_ENOMEM, "IFC block table exceeds the shared memory of one SM");
+    // The level-1 table of a row (nblk x 9 complex numbers, 144 bytes per contraction block) lives in shared memory: with
+    // the queues of the fused kernel that caps the list at about 1,400 blocks (include/fourphonon.h, "Limits").
+    auto too_many_blocks = [&](size_t need) {
+        return fail(ctx, FP_ENOMEM, "IFC" + std::to_string(order) + " list has " + std::to_string(f.nblk) + " contraction blocks (atomA, atomB, dR): "
+                    "its per-row table needs " + std::to_string(need) + " bytes of shared memory, more than the 226 KB of one SM "
+                    "(limit about 1,400 blocks)");
+    };
+    if (rates_smem_bytes(d, f) > 227 * 1024 - 1024) return too_many_blocks(rates_smem_bytes(d, f));
 
     // ---- scratch budget: per-target arrays for a super-chunk of targets ------------------------------------------------
     const size_t scratch_all = ctx->ws_bytes - ctx->resident;
@@ -563,8 +652,7 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
         const size_t rowbytes = (size_t)f.nblk * 9 * sizeof(double2);
         ge = (int)std::max<size_t>(1, std::min<size_t>((size_t)rbound, FP_EVAL_TILE_BYTES / rowbytes));
         if (order == 4 && ge >= njcap) ge = ge / njcap * njcap;      // whole targets: their rows share the level-0 loads
-        if (eval_smem_bytes(d, f, ge) > 227 * 1024 - 1024)
-            return fail(ctx, FP_ENOMEM, "IFC block table exceeds the shared memory of one SM");
+        if (eval_smem_bytes(d, f, ge) > 227 * 1024 - 1024) return too_many_blocks(eval_smem_bytes(d, f, ge));
     }
     const size_t scratch = split ? scratch_all - list_region - 4096 : scratch_all;
     const size_t pre_per_target = (order == 3 ? (size_t)f.nblk * 9 : (size_t)f.n * 27) * sizeof(double2);
@@ -812,6 +900,9 @@ int fp_set_symmetry(fp_ctx *ctx, int on) { if (!ctx) return FP_EINVAL; ctx->use_
 int fp_get_symmetry(const fp_ctx *ctx) {
     return ctx ? ((ctx->use_sym && ctx->sym23 ? 1 : 0) | (ctx->use_sym && ctx->sym34 ? 2 : 0)) : FP_EINVAL;
 }
+
+int fp_set_target_symmetry(fp_ctx *ctx, int on) { if (!ctx) return FP_EINVAL; ctx->use_trs = on != 0; return FP_OK; }
+int fp_get_target_symmetry(const fp_ctx *ctx) { return ctx ? (ctx->use_trs && ctx->trs_ok ? 1 : 0) : FP_EINVAL; }
 
 int fp_set_prefilter(fp_ctx *ctx, int on) {
     if (!ctx) return FP_EINVAL;

@@ -110,6 +110,11 @@ struct fp_ctx {
     int path = FP_PATH_AUTO;      // fp_set_path
     bool sym34 = false, sym23 = false;   // IFC4 / IFC3 is symmetric under the exchange of its last two legs (fp_setup)
     bool use_sym = true;          // fp_set_symmetry
+    // time reversal (fp_set_target_symmetry): the mode arrays satisfy omega(-q,j) = omega(q,j), v(-q,j) = -v(q,j),
+    // e(-q,j) = conj(e(q,j)) bit for bit (checked by fp_setup), so targets (q,j) and (-q,j) have the same rates and the
+    // driver evaluates one of each pair (targets only in the irreducible part, N_list)
+    bool trs_ok = false, use_trs = true;
+    std::vector<int32_t> qpartner;   // N: index of -q
     bool pf_saved = false;        // fp_set_prefilter(ctx, 0) is in effect; the constants of fp_setup are kept here:
     float sv_pfK1 = 0, sv_pfC2 = 0, sv_pfNmax = 0, sv_pfW = 0, sv_gfC = 0, sv_gfD = 0, sv_gfW = 0;
     cudaStream_t side = nullptr;  // second stream of the split path: the enumerator of chunk k+1 runs beside the

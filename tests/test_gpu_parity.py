@@ -206,12 +206,14 @@ def test_small_scratch_splits_targets_and_gives_identical_results(fp):
     for path in PATHS(fp):                                            # chunking never changes a row's arithmetic
         with fp.Context.from_inputs(inp, scratch_bytes=256 << 20) as big:
             big.set_path(path)
+            big.set_target_symmetry(False)
             big.profile_enable(True)
             g, w, c = big.rates4(t)
             n_big = big.profile_get().n_rates
             assert n_big == 1 or path != fp.FP_PATH_FUSED
         with fp.Context.from_inputs(inp, scratch_bytes=512 << 10) as small:
             small.set_path(path)
+            small.set_target_symmetry(False)                          # (the candidate count below is that of all 24 targets)
             small.profile_enable(True)
             gs, ws, cs = small.rates4(t)
             p = small.profile_get()
@@ -388,6 +390,7 @@ def test_pair_symmetry_of_the_4ph_channels(fp):
         with fp.Context.from_inputs(inp, scratch_bytes=256 << 20) as ctx:
             ctx.set_path(fp.FP_PATH_SPLIT_SERIAL)
             ctx.set_symmetry(on)
+            ctx.set_target_symmetry(False)
             assert ctx.get_symmetry() == on
             ctx.profile_enable(True)
             res[on] = ctx.rates4(t)
@@ -430,3 +433,57 @@ def test_asymmetric_ifc_disables_the_pair_symmetry(fp):
     with fp.Context.from_inputs(inp, scratch_bytes=64 << 20) as ctx:
         assert ctx.get_symmetry_mask() == 0
     check3(fp, inp, inp.targets3[::5])
+
+
+def test_time_reversal_reuse_over_targets(fp):
+    """fp_setup finds the generated mode arrays time-reversal symmetric bit for bit (fp_inputs sets e(-q) = conj(e(q)),
+    v(-q) = -v(q), reading 17); fp_rates3 / full-range fp_rates4 then evaluate one target of each {(q,j), (-q,j)} pair.
+    Counts must not change at all, rates only by rounding order; about half of the 3ph work is done; a partial q' range
+    does not use it; a mode array that breaks the symmetry turns it off -- and every variant still matches the oracle."""
+    inp = fp_inputs.make_tiny("diamond", mesh=(4, 3, 3))
+    orc = _oracle(inp)
+    og3, ow3, oc3 = orc.rates3(inp.targets3)
+    res = {}
+    for on in (True, False):
+        with fp.Context.from_inputs(inp, scratch_bytes=256 << 20) as ctx:
+            ctx.set_target_symmetry(on)
+            assert ctx.get_target_symmetry() == on
+            ctx.profile_enable(True)
+            res[on] = ctx.rates3(inp.targets3) + (ctx.profile_get().evaluated,)
+    (g1, w1, c1, e1), (g0, w0, c0, e0) = res[True], res[False]
+    assert np.array_equal(c1, c0) and np.array_equal(c1, oc3)
+    assert e1 < 0.62 * e0
+    assert np.allclose(g1, g0, rtol=1e-12, atol=1e-13 * np.abs(g0).max())
+    assert_rates_close(g1, og3, "Gamma3 (time reversal)")
+    assert_rates_close(w1, ow3, "WP3 (time reversal)")
+    # 4ph: all branches of a q-point and of its partner -q, whole q' range (reuse) and a partial range (none)
+    N1, N2, N3 = (int(x) for x in inp.mesh)
+    q = 1 + N1 * (2 + N2 * 1)
+    qm = (N1 - 1) % N1 + N1 * ((N2 - 2) % N2 + N2 * ((N3 - 1) % N3))
+    t4 = np.array([q * inp.nb + j for j in range(inp.nb)] + [qm * inp.nb + j for j in range(inp.nb)], dtype=np.int32)
+    og4, ow4, oc4 = orc.rates4(t4)
+    ogp, owp, ocp = orc.rates4(t4, 3, 9)
+    with fp.Context.from_inputs(inp, scratch_bytes=256 << 20) as ctx:
+        ctx.profile_enable(True)
+        g, w, c = ctx.rates4(t4)
+        ev_full = ctx.profile_get().evaluated
+        gp, wp_, cp = ctx.rates4(t4, 3, 9)
+        ctx.set_target_symmetry(False)
+        ctx.profile_reset()
+        g_, w_, c_ = ctx.rates4(t4)
+        assert ctx.profile_get().evaluated == 2 * ev_full
+    assert np.array_equal(c, oc4) and np.array_equal(c_, oc4) and np.array_equal(cp, ocp)
+    assert np.array_equal(c[:inp.nb], c[inp.nb:])
+    assert_rates_close(g, og4, "Gamma4 (time reversal)")
+    assert_rates_close(gp, ogp, "Gamma4 (partial q' range)")
+    assert np.allclose(g, g_, rtol=1e-12, atol=1e-13 * np.abs(g_).max())
+    # broken symmetry: one eigenvector component of one mode changed by an ulp-scale amount
+    import copy
+    bad = copy.copy(inp)
+    bad.eig = inp.eig.copy()
+    bad.eig.reshape(-1)[5 * inp.nb * inp.nb * 2 + 3] *= (1.0 + 1e-12)
+    with fp.Context.from_inputs(bad, scratch_bytes=256 << 20) as ctx:
+        assert not ctx.get_target_symmetry()
+        gb, wb, cb = ctx.rates3(inp.targets3)
+    assert np.array_equal(cb, oc3)
+    assert np.allclose(gb, og3, rtol=1e-9, atol=1e-9 * np.abs(og3).max())
