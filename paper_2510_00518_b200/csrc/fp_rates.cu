@@ -1,15 +1,8 @@
-// fp_rates.cu -- the rate kernels of the FourPhonon hot path (SURVEY.md §8(a) rows a2/a3 + a5/a6 + a7) and the
-// per-target pre-contraction.
+// fp_rates.cu -- the per-target pre-contraction and the fused rate kernel of the FourPhonon hot path (SURVEY.md §8(a)
+// rows a2/a3 + a5/a6 + a7).
 //
 //   k_pre3/k_pre4  per-target level-0 contraction of the IFC list with the target eigenvector
-//   split path (default): Algorithm 3 -> Algorithm 4 of the paper, both on the device
-//     k_enum       one CTA per row (3ph: (target, channel); 4ph: (target, channel, lambda')).  Each warp enumerates its
-//                  share of the row's candidates (momentum modulo the mesh PAPER.md:155,288), filters them with the
-//                  two-stage FP32 pre-filter, takes the window decision in the pinned FP64 arithmetic
-//                  of SURVEY.md §8(c) step 3, computes the row-independent part of the weight and
-//                  ballot-compacts the allowed processes into its list slot (16 bytes per process)
-//     k_eval       one CTA per row: matrix element of every listed process (compute_Vp), two processes
-//                  per lane against one pass over the row's contraction blocks, accumulation
+//   group path (default): k_enum_g -> per-row process lists -> k_eval_g, in fp_group.cu
 //   fused path (small scratch, or a list slot that filled up)
 //     k_rates      one CTA per row does all of the above; the process lists live and die in shared memory
 //
