@@ -149,6 +149,18 @@ int fp_list3(fp_ctx *ctx, int32_t target, int32_t channel, int32_t *pairs, int64
 int fp_list4(fp_ctx *ctx, int32_t target, int32_t channel, int32_t qp, int32_t *triples, int64_t cap, int64_t *n,
              void *stream);
 
+/* Per-process terms (an iterative BTE solver needs the rate of every process,
+ * not only the per-mode sums).  The same lists as fp_list3 / fp_list4 -- full rectangular domain, no symmetry reuse --
+ * with, for every process p, its contribution to the rate of the target in that channel:
+ *   gamma_p = (C3/N) s_ch WP_p |V3_p|^2   resp.   (C4/N^2) s_ch WP_p |V4_p|^2      (1/ps; s_ch = 1, 1/2 | 1/2, 1/2, 1/6)
+ * from the same pinned window decision, weights and level-2 contraction as fp_rates3 / fp_rates4, so that
+ * sum_p gamma_p = Gamma^{ch}(target) (over q' = qp for fp_terms4) up to summation order.
+ *   pairs / triples  HOST cap*2 / cap*3 int32 (nullable if cap == 0);  gamma_p  HOST cap doubles
+ *   *n receives the number of allowed processes (may exceed cap; only cap entries are written).                       */
+int fp_terms3(fp_ctx *ctx, int32_t target, int32_t channel, int32_t *pairs, double *gamma_p, int64_t cap, int64_t *n, void *stream);
+int fp_terms4(fp_ctx *ctx, int32_t target, int32_t channel, int32_t qp, int32_t *triples, double *gamma_p, int64_t cap, int64_t *n,
+              void *stream);
+
 /* Execution path of fp_rates3 / fp_rates4 (same results bit for bit in counts, within rounding order in rates):
  *   FP_PATH_SPLIT_SERIAL  enumerator kernel (pre-filter, pinned FP64 decision, weights) -> process lists in half of the
  *                  scratch region -> evaluator kernel (|V|^2, row sums): Algorithms 3 and 4, both on

@@ -28,7 +28,7 @@ _SOURCES = ["fp_kernels.cu", "fp_rates.cu", "fp_group.cu", "fp_host.cu"]
 # every symbol include/fourphonon.h declares (tests check that the built library exports all of them)
 EXPORTED_SYMBOLS = [
     "fp_workspace_bytes", "fp_setup", "fp_rates3", "fp_rates4", "fp_kappa_rta", "fp_list3", "fp_list4",
-    "fp_set_path", "fp_set_symmetry", "fp_get_symmetry", "fp_set_target_symmetry", "fp_get_target_symmetry", "fp_set_prefilter", "fp_profile_enable", "fp_profile_reset", "fp_profile_get", "fp_probe_fp64_tflops", "fp_probe_dmma_tflops", "fp_constants",
+    "fp_terms3", "fp_terms4", "fp_set_path", "fp_set_symmetry", "fp_get_symmetry", "fp_set_target_symmetry", "fp_get_target_symmetry", "fp_set_prefilter", "fp_profile_enable", "fp_profile_reset", "fp_profile_get", "fp_probe_fp64_tflops", "fp_probe_dmma_tflops", "fp_constants",
     "fp_last_error", "fp_version", "fp_destroy",
 ]
 
@@ -130,6 +130,10 @@ def load_library():
     lib.fp_list3.argtypes = [vp, i32, i32, vp, i64, C.POINTER(i64), vp]
     lib.fp_list4.restype = C.c_int
     lib.fp_list4.argtypes = [vp, i32, i32, i32, vp, i64, C.POINTER(i64), vp]
+    lib.fp_terms3.restype = C.c_int
+    lib.fp_terms3.argtypes = [vp, i32, i32, vp, vp, i64, C.POINTER(i64), vp]
+    lib.fp_terms4.restype = C.c_int
+    lib.fp_terms4.argtypes = [vp, i32, i32, i32, vp, vp, i64, C.POINTER(i64), vp]
     lib.fp_set_path.restype = C.c_int
     lib.fp_set_path.argtypes = [vp, C.c_int]
     lib.fp_set_symmetry.restype = C.c_int
@@ -388,6 +392,29 @@ class Context:
             self._check(self.lib.fp_list4(self.ctx, int(target), int(channel), int(qp), out.ctypes.data, n.value,
                                           C.byref(n), _stream_ptr(stream)))
         return out[:n.value]
+
+    def terms3(self, target, channel, stream=None):
+        """fp_terms3: the 3ph process list of one target and channel and each process's contribution to Gamma."""
+        n = C.c_int64(0)
+        with self._torch.cuda.device(self.device):
+            self._check(self.lib.fp_terms3(self.ctx, int(target), int(channel), None, None, 0, C.byref(n), _stream_ptr(stream)))
+            out = np.zeros((max(n.value, 1), 2), dtype=np.int32)
+            g = np.zeros(max(n.value, 1), dtype=np.float64)
+            self._check(self.lib.fp_terms3(self.ctx, int(target), int(channel), out.ctypes.data, g.ctypes.data, n.value,
+                                           C.byref(n), _stream_ptr(stream)))
+        return out[:n.value], g[:n.value]
+
+    def terms4(self, target, channel, qp, stream=None):
+        """fp_terms4: the 4ph process list of one target, channel and q-prime and each process's contribution to Gamma."""
+        n = C.c_int64(0)
+        with self._torch.cuda.device(self.device):
+            self._check(self.lib.fp_terms4(self.ctx, int(target), int(channel), int(qp), None, None, 0, C.byref(n),
+                                           _stream_ptr(stream)))
+            out = np.zeros((max(n.value, 1), 3), dtype=np.int32)
+            g = np.zeros(max(n.value, 1), dtype=np.float64)
+            self._check(self.lib.fp_terms4(self.ctx, int(target), int(channel), int(qp), out.ctypes.data, g.ctypes.data,
+                                           n.value, C.byref(n), _stream_ptr(stream)))
+        return out[:n.value], g[:n.value]
 
     def set_path(self, path: int):
         """FP_PATH_AUTO / FP_PATH_FUSED / FP_PATH_SPLIT / FP_PATH_SPLIT_SERIAL (include/fourphonon.h)."""

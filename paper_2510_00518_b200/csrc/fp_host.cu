@@ -839,7 +839,7 @@ int fp_kappa_rta(fp_ctx *ctx, const double *gamma_total, double *kappa, fp_memlo
 
 // ---- debug list export -------------------------------------------------------------------------------------------------
 static int list_driver(fp_ctx *ctx, int order, int32_t target, int32_t channel, int32_t qp, int32_t *out, int64_t cap,
-                       int64_t *n, cudaStream_t st) {
+                       int64_t *n, cudaStream_t st, double *terms = nullptr) {
     if (!ctx || !n) return FP_EINVAL;
     const FpDev &d = ctx->d;
     if (!(order == 3 ? ctx->has3 : ctx->has4)) return fail(ctx, FP_ESTATE, "no IFC list of this order was given to fp_setup");
@@ -877,6 +877,19 @@ static int list_driver(fp_ctx *ctx, int order, int32_t target, int32_t channel, 
     *n = ho[re] - ho[rb];
     const int64_t ncopy = std::min(*n, cap);
     if (ncopy > 0) CU(cudaMemcpyAsync(out, dec, ncopy * w * 4, cudaMemcpyDeviceToHost, st));
+    if (terms && *n > 0) {                                            // per-process terms: level 0 of the target, then k_terms
+        const IfcDev &f = order == 3 ? ctx->i3 : ctx->i4;
+        if (rates_smem_bytes(d, f) > 227 * 1024 - 1024) return fail(ctx, FP_ENOMEM, "IFC block table exceeds the shared memory of one SM");
+        double2 *pre = sc.take<double2>(order == 3 ? (size_t)f.nblk * 9 : (size_t)f.n * 27);
+        double *gp = sc.take<double>(*n);
+        if (!pre || !gp) return fail(ctx, FP_ENOMEM, "scratch");
+        if (order == 3) launch_pre3(d, f, d_t, 1, pre, st); else launch_pre4(d, f, d_t, 1, pre, st);
+        const double sym = order == 3 ? (channel == 0 ? 1.0 : 0.5) : (channel == 2 ? 1.0 / 6.0 : 0.5);
+        const double c_over_n = order == 3 ? const_c3() / (double)d.N : const_c4() / ((double)d.N * (double)d.N);
+        RowArgs rr = ra; rr.row0 = rb;
+        CU(launch_terms(order, d, f, rr, re - rb, pre, offs, ho[rb], list + ho[rb], c_over_n * sym, gp, st));
+        if (ncopy > 0) CU(cudaMemcpyAsync(terms, gp, ncopy * 8, cudaMemcpyDeviceToHost, st));
+    }
     CU(cudaStreamSynchronize(st));
     return FP_OK;
 }
@@ -894,6 +907,16 @@ int fp_set_path(fp_ctx *ctx, int path) {
     if (!ctx || path < FP_PATH_AUTO || path > FP_PATH_SPLIT_SERIAL) return ctx ? fail(ctx, FP_EINVAL, "unknown path") : FP_EINVAL;
     ctx->path = path;
     return FP_OK;
+}
+
+int fp_terms3(fp_ctx *ctx, int32_t target, int32_t channel, int32_t *pairs, double *gamma_p, int64_t cap, int64_t *n, void *stream) {
+    if (!gamma_p && cap > 0) return ctx ? fail(ctx, FP_EINVAL, "null gamma_p") : FP_EINVAL;
+    return list_driver(ctx, 3, target, channel, 0, pairs, cap, n, (cudaStream_t)stream, gamma_p);
+}
+int fp_terms4(fp_ctx *ctx, int32_t target, int32_t channel, int32_t qp, int32_t *triples, double *gamma_p, int64_t cap, int64_t *n,
+              void *stream) {
+    if (!gamma_p && cap > 0) return ctx ? fail(ctx, FP_EINVAL, "null gamma_p") : FP_EINVAL;
+    return list_driver(ctx, 4, target, channel, qp, triples, cap, n, (cudaStream_t)stream, gamma_p);
 }
 
 int fp_set_symmetry(fp_ctx *ctx, int on) { if (!ctx) return FP_EINVAL; ctx->use_sym = on != 0; return FP_OK; }

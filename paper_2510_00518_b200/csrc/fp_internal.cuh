@@ -140,6 +140,10 @@ void launch_pre4(const FpDev &d, const IfcDev &f, const int32_t *targets, int64_
 cudaError_t launch_rates(int order, const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const double2 *pre,
                          double2 *partial, uint32_t *counts, bool only_flagged, cudaStream_t st);
 size_t rates_smem_bytes(const FpDev &d, const IfcDev &f);
+// per-process terms of explicit lists (fp_terms3 / fp_terms4): row r of the launch is ra.row0 + blockIdx.x
+cudaError_t launch_terms(int order, const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const double2 *pre,
+                         const int64_t *offsets, int64_t list_base, const uint32_t *list, double scale, double *gamma_p,
+                         cudaStream_t st);
 // group path (fp_group.cu): group enumerator -> per-row process lists in the scratch -> tile evaluator
 #define FP_GROUP_RMAX 64          // rows of one enumerator group (they share the scan of the two free legs)
 int64_t enum_slot_entries(const FpDev &d);        // entries of one (row, warp) list slot that can never overflow

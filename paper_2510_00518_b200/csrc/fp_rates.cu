@@ -395,6 +395,38 @@ __global__ void __launch_bounds__(RT, RATES_MINB) k_rates(FpDev d, IfcDev f, Row
 // ---------------------------------------------------------------------------------------------------------------------
 // launchers
 // ---------------------------------------------------------------------------------------------------------------------
+// ---------------------------------------------------------------------------------------------------------------------
+// per-process terms (an iterative solver needs the rate of every single process)
+// ---------------------------------------------------------------------------------------------------------------------
+// One CTA per row of an explicit process list (k_count -> k_scan -> k_fill, fp_kernels.cu): the row's tables as in
+// k_rates, then every listed process through the same eval_process -- pinned decision, weights, level-2 contraction --
+// whose result is stored instead of summed: gamma_p = scale * WP_p |V_p|^2, scale = (C/N^k) x the channel's symmetry weight.
+template <int ORDER>
+__global__ void __launch_bounds__(RT) k_terms(FpDev d, IfcDev f, RowArgs ra, const double2 *pre, const int64_t *offsets,
+                                              int64_t list_base, const uint32_t *list, double scale, double *gamma_p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int64_t r = ra.row0 + blockIdx.x;
+    const int64_t beg = offsets[r] - list_base, cnt = offsets[r + 1] - offsets[r];
+    if (cnt == 0) return;
+    const Row row = make_row<ORDER>(d, ra, r);
+    BlkSmem bs;
+    RowWeights rw;
+    setup_row_tables<ORDER>(d, f, row, pre, smem_raw, bs, rw);
+    for (int64_t i0 = 0; i0 < cnt; i0 += RT) {
+        const int64_t i = i0 + threadIdx.x;
+        const bool act = i < cnt;
+        const uint32_t code = list[beg + (act ? i : 0)];
+        const int p = (int)(code / (uint32_t)d.nb), jb = (int)(code - (uint32_t)p * (uint32_t)d.nb);
+        const int qx = p / d.nb, ja = p - qx * d.nb;
+        const int ql = q_index(d, q_add(d, row.qb, row.s2, unpack_qc(d.qc[qx])));
+        double sG = 0.0, sW = 0.0;
+        unsigned c = 0;
+        eval_process<ORDER, 0>(d, bs, row, rw, make_uint2(((uint32_t)qx << 6) | (uint32_t)ja, ((uint32_t)ql << 6) | (uint32_t)jb), act, sG,
+                               sW, c);
+        if (act) gamma_p[beg + i] = scale * sG;
+    }
+}
+
 void launch_pre3(const FpDev &d, const IfcDev &f, const int32_t *targets, int64_t nt, double2 *mhat, cudaStream_t st) {
     if (nt > 0) k_pre3<<<(unsigned)nt, 256, 0, st>>>(d, f, targets, mhat);
 }
@@ -405,6 +437,23 @@ void launch_pre4(const FpDev &d, const IfcDev &f, const int32_t *targets, int64_
 static size_t tables_smem_bytes(const FpDev &d, const IfcDev &f) {
     return (size_t)f.nblk * 9 * sizeof(double2) + (size_t)d.L * sizeof(double2) + (size_t)d.nb * sizeof(double2) +
            (size_t)f.nblk * sizeof(int4) + (size_t)((d.nat * d.nat + 1 + 3) & ~3) * sizeof(int);
+}
+cudaError_t launch_terms(int order, const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const double2 *pre,
+                         const int64_t *offsets, int64_t list_base, const uint32_t *list, double scale, double *gamma_p,
+                         cudaStream_t st) {
+    if (nrows <= 0) return cudaSuccess;
+    const size_t smem = (tables_smem_bytes(d, f) + 15) & ~(size_t)15;
+    static SmemGrant g3, g4;
+    if (order == 3) {
+        cudaError_t e = opt_in_smem(k_terms<3>, smem, g3);
+        if (e != cudaSuccess) return e;
+        k_terms<3><<<(unsigned)nrows, RT, smem, st>>>(d, f, ra, pre, offsets, list_base, list, scale, gamma_p);
+    } else {
+        cudaError_t e = opt_in_smem(k_terms<4>, smem, g4);
+        if (e != cudaSuccess) return e;
+        k_terms<4><<<(unsigned)nrows, RT, smem, st>>>(d, f, ra, pre, offsets, list_base, list, scale, gamma_p);
+    }
+    return cudaGetLastError();
 }
 size_t rates_smem_bytes(const FpDev &d, const IfcDev &f) {
     size_t b = tables_smem_bytes(d, f) + (size_t)(RW * QCAP + RW * 32) * sizeof(uint2) + (size_t)(RW * PCAP) * sizeof(uint32_t);

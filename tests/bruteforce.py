@@ -233,3 +233,41 @@ def list4_bruteforce(inp, lam, ch, scale=1.0, ncut=2.0, T=300.0):
                     for j2, j3 in zip(*np.nonzero(near)):
                         margin[(q1 * nb + j1, q2 * nb + int(j2), q3 * nb + int(j3))] = abs(d[j2, j3]) - ncut * sig[j2, j3]
     return out, margin, wp * (1.0 / 6.0 if ch == 2 else 0.5) / N ** 2
+
+
+def term4_dense(inp, lam, ch, triple, scale=1.0, T=300.0):
+    """Contribution of ONE 4ph process (lam; lam1, lam2, lam3) of channel ch to Gamma(lam), in plain numpy: the dense-Fourier
+    matrix element (v4_dense), PAPER.md:163's Gaussian with the adaptive sigma of the last two legs (item 2), the "/f"
+    occupation form (item 5), C4/N^2 and the symmetry weight (items 6)."""
+    c4 = si_chain_constants()[1]
+    nb, N = inp.nb, inp.nq
+    lam1, lam2, lam3 = (int(x) for x in triple)
+    s1, s2 = ((1, 1), (1, -1), (-1, -1))[ch]
+    w = inp.omega.reshape(-1)
+    v = inp.vg.reshape(-1, 3)
+    Bm = recip_cart(inp.crystal.lattvec) / np.asarray(inp.mesh, float)[:, None]
+    sig = scale * np.sqrt((((v[lam2] - v[lam3]) @ Bm.T) ** 2).sum() / 6.0)
+    d = w[lam] + s1 * w[lam1] + s2 * w[lam2] - w[lam3]
+    g = np.exp(-(d / sig) ** 2) / (sig * np.sqrt(np.pi))
+    f0, f1, f2, f3 = (be(w[x], T) for x in (lam, lam1, lam2, lam3))
+    occ = ((1 + f1) if s1 > 0 else f1) * ((1 + f2) if s2 > 0 else f2) * f3 / f0
+    V = v4_dense(inp, lam, lam1, lam2, lam3, s1, s2)
+    return c4 / N ** 2 * (1.0 / 6.0 if ch == 2 else 0.5) * occ * g / (w[lam] * w[lam1] * w[lam2] * w[lam3]) * abs(V) ** 2
+
+
+def term3_dense(inp, lam, ch, pair, scale=1.0, T=300.0):
+    """The same for one 3ph process (lam; lam1, lam2): sigma from v' - v'', occupation f' - f'' (+) or f' + f'' + 1 (-)."""
+    c3 = si_chain_constants()[0]
+    N = inp.nq
+    lam1, lam2 = (int(x) for x in pair)
+    s = 1 if ch == 0 else -1
+    w = inp.omega.reshape(-1)
+    v = inp.vg.reshape(-1, 3)
+    Bm = recip_cart(inp.crystal.lattvec) / np.asarray(inp.mesh, float)[:, None]
+    sig = scale * np.sqrt((((v[lam1] - v[lam2]) @ Bm.T) ** 2).sum() / 6.0)
+    d = w[lam] + s * w[lam1] - w[lam2]
+    g = np.exp(-(d / sig) ** 2) / (sig * np.sqrt(np.pi))
+    f1, f2 = be(w[lam1], T), be(w[lam2], T)
+    occ = (f1 - f2) if s > 0 else (f1 + f2 + 1.0)
+    V = v3_dense(inp, lam, lam1, lam2, s)
+    return c3 / N * (1.0 if ch == 0 else 0.5) * occ * g / (w[lam] * w[lam1] * w[lam2]) * abs(V) ** 2

@@ -487,3 +487,33 @@ def test_time_reversal_reuse_over_targets(fp):
         gb, wb, cb = ctx.rates3(inp.targets3)
     assert np.array_equal(cb, oc3)
     assert np.allclose(gb, og3, rtol=1e-9, atol=1e-9 * np.abs(og3).max())
+
+
+def test_per_process_terms(fp):
+    """fp_terms3 / fp_terms4: the process lists of fp_list3/4 with each process's
+    contribution to Gamma.  The terms sum to the oracle's Gamma of that target, channel (and q'), their number is the
+    oracle's count, and sampled terms equal an independent numpy evaluation (dense-Fourier matrix element x weights; a
+    matrix element that vanishes by symmetry is rounding noise on both sides, hence the floor of 1e-14 of the largest term)."""
+    from . import bruteforce as bf
+    inp = fp_inputs.make_tiny("diamond", mesh=(3, 3, 3))
+    orc = _oracle(inp)
+    rng = np.random.default_rng(5)
+    with fp.Context.from_inputs(inp, scratch_bytes=256 << 20) as ctx:
+        for lam in (7, 40, 101):
+            og, ow, oc = orc.rates3(np.array([lam], dtype=np.int32))
+            for ch in (0, 1):
+                pairs, g = ctx.terms3(lam, ch)
+                assert len(g) == int(oc[0, ch]) and np.array_equal(pairs, ctx.list3(lam, ch))
+                assert abs(g.sum() - og[0, ch]) <= 1e-9 * abs(og[0, ch])
+                for i in rng.choice(len(g), size=min(4, len(g)), replace=False):
+                    ref = bf.term3_dense(inp, lam, ch, pairs[i])
+                    assert abs(g[i] - ref) <= 1e-8 * abs(ref) + 1e-14 * g.max(), (lam, ch, pairs[i], g[i], ref)
+        for lam, qp in ((8, 5), (61, 20), (20, 3)):
+            og, ow, oc = orc.rates4(np.array([lam], dtype=np.int32), qp, qp + 1)
+            for ch in (0, 1, 2):
+                triples, g = ctx.terms4(lam, ch, qp)
+                assert len(g) == int(oc[0, ch]) and np.array_equal(triples, ctx.list4(lam, ch, qp))
+                assert abs(g.sum() - og[0, ch]) <= 1e-9 * max(abs(og[0, ch]), 1e-10 * np.abs(og).max())   # (floor: DESIGN.md §5.2)
+                for i in rng.choice(len(g), size=min(3, len(g)), replace=False):
+                    ref = bf.term4_dense(inp, lam, ch, triples[i])
+                    assert abs(g[i] - ref) <= 1e-8 * abs(ref) + 1e-14 * np.abs(og).max(), (lam, ch, triples[i], g[i], ref)
