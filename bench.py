@@ -187,6 +187,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--path", choices=["auto", "fused", "split", "split-serial"], default="auto",
                     help="execution path of fp_rates3/4 (fp_set_path); auto = split when the scratch holds the lists")
+    ap.add_argument("--precision", choices=["fp64", "mixed"], default="fp64",
+                    help="mixed = fp_set_precision(FP_PREC_MIXED): level-2 contraction in FP32 (not the headline: fails the 1e-9 bar)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -215,6 +217,8 @@ def main():
     for inp, t3, t4 in jobs:
         ctx = fp.Context.from_inputs(inp, scratch_bytes=scratch, device=dev)
         ctx.set_path(path_id)
+        if args.precision == "mixed":
+            ctx.set_precision(fp.FP_PREC_MIXED)
         ctxs.append(ctx)
         dev_targets.append((None if t3 is None else torch.from_numpy(np.ascontiguousarray(t3)).to(dev),
                             None if t4 is None else torch.from_numpy(np.ascontiguousarray(t4)).to(dev)))
@@ -241,6 +245,8 @@ def main():
         for inp, t3, t4 in jobs:
             with fp.Context.from_inputs(inp, scratch_bytes=scratch, device=dev) as ctx:
                 ctx.set_path(path_id)
+                if args.precision == "mixed":
+                    ctx.set_precision(fp.FP_PREC_MIXED)
                 h2d += inp.omega.nbytes + inp.eig.nbytes + inp.vg.nbytes
                 for ifc in (inp.ifc3, inp.ifc4):
                     if ifc is not None:
@@ -358,7 +364,8 @@ def main():
                 "path": "split" if split else "fused", "list_slot_overflows_per_step": overflows}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64" if args.precision == "fp64" else "f32 level-2 contraction, f64 decision/weights/sums (NOT the headline)",
             "data": "synthetic",
             "config": {"workload": workload_name(args.config), "step": "fp_rates3 + fp_rates4 + fp_kappa_rta",
                        "processes_4ph_per_step": n4, "processes_3ph_per_step": n3, "processes_counted_in_value": counted, "parallelism": f"replicas x{world}",

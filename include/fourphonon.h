@@ -197,6 +197,17 @@ int fp_get_symmetry(const fp_ctx *ctx);
 int fp_set_target_symmetry(fp_ctx *ctx, int on);
 int fp_get_target_symmetry(const fp_ctx *ctx);
 
+/* Mixed precision ("FP32 where accuracy allows").  FP_PREC_MIXED evaluates the
+ * per-process matrix element -- the level-2 contraction of the group path's evaluator, > 95 % of the FP64 work -- in FP32
+ * (eigenvectors, the per-row table Mhat and the phases rounded to FP32, FP32 FMAs); the window decision, hence the counts,
+ * the weights WP, levels 0 and 1 of the contraction and all sums stay FP64.  Gamma then carries the FP32 rounding of
+ * |V|^2 (relative error ~1e-6 per process, less in the sums): it does NOT meet the 1e-9 parity bar and is off by
+ * default.  nat <= 2 only (the generic evaluator and the fused path ignore the switch).                              */
+#define FP_PREC_FP64  0
+#define FP_PREC_MIXED 1
+int fp_set_precision(fp_ctx *ctx, int mode);
+int fp_get_precision(const fp_ctx *ctx);
+
 /* Self-check of the FP32 pre-filter (DESIGN.md §5.2 claims it admits a superset of the candidates the pinned FP64 window
  * decision of PAPER.md:163,293 allows, so that counts and rates never depend on it).  fp_set_prefilter(ctx, 0) disables
  * every FP32 test -- each candidate then takes the pinned FP64 decision, 10-50x slower -- and fp_set_prefilter(ctx, 1)

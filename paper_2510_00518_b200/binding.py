@@ -18,6 +18,7 @@ import numpy as np
 
 FP_OK, FP_EINVAL, FP_ENOMEM, FP_ECUDA, FP_ESTATE = 0, -1, -2, -3, -4
 FP_PATH_AUTO, FP_PATH_FUSED, FP_PATH_SPLIT, FP_PATH_SPLIT_SERIAL = 0, 1, 2, 3
+FP_PREC_FP64, FP_PREC_MIXED = 0, 1
 FP_MEM_HOST, FP_MEM_DEVICE = 0, 1
 
 _PKG = Path(__file__).resolve().parent
@@ -28,7 +29,7 @@ _SOURCES = ["fp_kernels.cu", "fp_rates.cu", "fp_group.cu", "fp_host.cu"]
 # every symbol include/fourphonon.h declares (tests check that the built library exports all of them)
 EXPORTED_SYMBOLS = [
     "fp_workspace_bytes", "fp_setup", "fp_rates3", "fp_rates4", "fp_kappa_rta", "fp_list3", "fp_list4",
-    "fp_terms3", "fp_terms4", "fp_set_path", "fp_set_symmetry", "fp_get_symmetry", "fp_set_target_symmetry", "fp_get_target_symmetry", "fp_set_prefilter", "fp_profile_enable", "fp_profile_reset", "fp_profile_get", "fp_probe_fp64_tflops", "fp_probe_dmma_tflops", "fp_constants",
+    "fp_terms3", "fp_terms4", "fp_set_path", "fp_set_symmetry", "fp_get_symmetry", "fp_set_target_symmetry", "fp_get_target_symmetry", "fp_set_precision", "fp_get_precision", "fp_set_prefilter", "fp_profile_enable", "fp_profile_reset", "fp_profile_get", "fp_probe_fp64_tflops", "fp_probe_dmma_tflops", "fp_constants",
     "fp_last_error", "fp_version", "fp_destroy",
 ]
 
@@ -144,6 +145,10 @@ def load_library():
     lib.fp_set_target_symmetry.argtypes = [vp, C.c_int]
     lib.fp_get_target_symmetry.restype = C.c_int
     lib.fp_get_target_symmetry.argtypes = [vp]
+    lib.fp_set_precision.restype = C.c_int
+    lib.fp_set_precision.argtypes = [vp, C.c_int]
+    lib.fp_get_precision.restype = C.c_int
+    lib.fp_get_precision.argtypes = [vp]
     lib.fp_set_prefilter.restype = C.c_int
     lib.fp_set_prefilter.argtypes = [vp, C.c_int]
     lib.fp_profile_enable.restype = C.c_int
@@ -431,6 +436,13 @@ class Context:
     def get_target_symmetry(self) -> bool:
         """True if fp_setup found the mode arrays time-reversal symmetric bit for bit and the reuse is on."""
         return self.lib.fp_get_target_symmetry(self.ctx) > 0
+
+    def set_precision(self, mode: int):
+        """fp_set_precision: FP_PREC_FP64 (default) or FP_PREC_MIXED (level-2 contraction in FP32; include/fourphonon.h)."""
+        self._check(self.lib.fp_set_precision(self.ctx, int(mode)))
+
+    def get_precision(self) -> int:
+        return int(self.lib.fp_get_precision(self.ctx))
 
     def set_prefilter(self, on: bool):
         """fp_set_prefilter: False disables every FP32 pre-filter test (self-check of the superset claim; slow)."""

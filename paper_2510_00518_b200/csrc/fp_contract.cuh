@@ -148,6 +148,44 @@ __device__ __forceinline__ void contract_process2(const FpDev &d, const BlkSmem 
         }
 }
 
+// Mixed precision (fp_set_precision): the same two-process contraction in FP32 -- Mhat, phases and both
+// eigenvectors rounded to FP32, FP32 FMAs.  NAT > 0 only.
+__device__ __forceinline__ void cfmaf(float2 &acc, float2 a, float2 b) {
+    acc.x = fmaf(a.x, b.x, acc.x);
+    acc.x = fmaf(-a.y, b.y, acc.x);
+    acc.y = fmaf(a.x, b.y, acc.y);
+    acc.y = fmaf(a.y, b.x, acc.y);
+}
+template <int NAT>
+__device__ __forceinline__ void contract_process2_f32(const FpDev &d, const BlkSmem &bs, const float2 *Mf, const float2 *phf,
+                                                      const float2 *A0, const float2 *B0, int3 q0, const float2 *A1,
+                                                      const float2 *B1, int3 q1, float2 &V0, float2 &V1) {
+    V0 = make_float2(0.f, 0.f); V1 = make_float2(0.f, 0.f);
+#pragma unroll
+    for (int a = 0; a < NAT; a++)
+#pragma unroll
+        for (int c = 0; c < NAT; c++) {
+            const int b1 = bs.seg[a * NAT + c + 1];
+            for (int b = bs.seg[a * NAT + c]; b < b1; b++) {
+                const int4 m = bs.meta[b];
+                const float2 p0 = phf[phase_idx(d, q0, m.y, m.z, m.w)], p1 = phf[phase_idx(d, q1, m.y, m.z, m.w)];
+                const float2 *M = Mf + 9 * b;
+                float2 u0 = make_float2(0.f, 0.f), u1 = make_float2(0.f, 0.f);
+#pragma unroll
+                for (int y = 0; y < 3; y++) {
+                    float2 t0 = make_float2(0.f, 0.f), t1 = make_float2(0.f, 0.f);
+#pragma unroll
+                    for (int x = 0; x < 3; x++) {
+                        const float2 mm = M[3 * x + y];
+                        cfmaf(t0, mm, A0[3 * a + x]); cfmaf(t1, mm, A1[3 * a + x]);
+                    }
+                    cfmaf(u0, t0, B0[3 * c + y]); cfmaf(u1, t1, B1[3 * c + y]);
+                }
+                cfmaf(V0, u0, p0); cfmaf(V1, u1, p1);
+            }
+        }
+}
+
 // The same for any atom count, every eigenvector component fetched once: the leg-A vectors of the two processes are
 // staged by the caller in shared memory (As[comp * 64 + 32 h], already offset by the lane: each lane reads back only
 // what it wrote), the loop runs atom-B-major with the three conj(e~_B) components of atom c in registers (those of

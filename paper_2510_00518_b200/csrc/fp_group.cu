@@ -408,10 +408,11 @@ struct EvalSmem {
     unsigned *accC;    // nw * ge        processes (both orderings of a listed pair count)
     unsigned char *rot;  // ge           rotation of the row's chunk deal (a property of the row alone)
     double2 *As;       // nw * nb * 64   generic atom count: leg-A eigenvectors of a warp's chunk, [component][process]
+    float2 *Mf, *phf;  // ge * nblk*9, L mixed precision: Mhat and the phases rounded to FP32
 };
 // nw = warps of the CTA; stage: the generic evaluator (NAT = 0) stages one eigenvector per process of every warp's chunk
-__host__ __device__ inline size_t eval_smem_layout(int ge, int nblk, int L, int nb, int nat, int NU, int nw, bool stage, EvalSmem *es,
-                                                   unsigned char *base) {
+__host__ __device__ inline size_t eval_smem_layout(int ge, int nblk, int L, int nb, int nat, int NU, int nw, bool stage, bool mixed,
+                                                   EvalSmem *es, unsigned char *base) {
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t r = o; o += (bytes + 15) & ~(size_t)15; return r; };
     const size_t oM = take((size_t)ge * nblk * 9 * sizeof(double2)), oph = take((size_t)L * sizeof(double2)),
@@ -421,7 +422,8 @@ __host__ __device__ inline size_t eval_smem_layout(int ge, int nblk, int L, int 
                  orf = take((size_t)ge * sizeof(double)), oro = take((size_t)ge * sizeof(long long)),
                  och = take((size_t)(ge + 1) * sizeof(int)), oaG = take((size_t)nw * ge * sizeof(double)),
                  oaW = take((size_t)nw * ge * sizeof(double)), oaC = take((size_t)nw * ge * sizeof(unsigned)),
-                 orot = take((size_t)ge), oAs = take(stage ? (size_t)nw * nb * 64 * sizeof(double2) : 0);
+                 orot = take((size_t)ge), oAs = take(stage ? (size_t)nw * nb * 64 * sizeof(double2) : 0),
+                 oMf = take(mixed ? (size_t)ge * nblk * 9 * sizeof(float2) : 0), ophf = take(mixed ? (size_t)L * sizeof(float2) : 0);
     if (es) {
         es->M = reinterpret_cast<double2 *>(base + oM); es->ph = reinterpret_cast<double2 *>(base + oph);
         es->e1 = reinterpret_cast<double2 *>(base + oe1); es->meta = reinterpret_cast<int4 *>(base + ometa);
@@ -430,6 +432,7 @@ __host__ __device__ inline size_t eval_smem_layout(int ge, int nblk, int L, int 
         es->chunk0 = reinterpret_cast<int *>(base + och); es->accG = reinterpret_cast<double *>(base + oaG);
         es->accW = reinterpret_cast<double *>(base + oaW); es->accC = reinterpret_cast<unsigned *>(base + oaC);
         es->rot = base + orot; es->As = reinterpret_cast<double2 *>(base + oAs);
+        es->Mf = reinterpret_cast<float2 *>(base + oMf); es->phf = reinterpret_cast<float2 *>(base + ophf);
     }
     return o;
 }
@@ -438,15 +441,16 @@ __host__ __device__ inline size_t eval_smem_layout(int ge, int nblk, int L, int 
 #define FP_EVAL_MINB 3
 #endif
 constexpr int GEN_WMAX = 8;                   // warps of a generic-evaluator CTA, at most (as many as the staging leaves room for)
-template <int ORDER, int NAT, bool PH8>
-__global__ void __launch_bounds__(NAT > 0 ? GT : GEN_WMAX * 32, NAT > 0 ? FP_EVAL_MINB : 1) k_eval_g(FpDev d, IfcDev f, GroupArgs ga, const double2 *pre, int64_t capw,
+// MIX: level-2 contraction in FP32 (fp_set_precision; NAT > 0 only)
+template <int ORDER, int NAT, bool MIX>
+__global__ void __launch_bounds__(NAT > 0 ? GT : GEN_WMAX * 32, NAT > 0 ? (MIX ? 4 : FP_EVAL_MINB) : 1) k_eval_g(FpDev d, IfcDev f, GroupArgs ga, const double2 *pre, int64_t capw,
                                                   const ListEnt *lists, const uint32_t *wcnt, int ge, int tiles_per_group,
                                                   double2 *partial, uint32_t *counts) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ int s_nitems;
     EvalSmem es;
     const int nthr = NAT > 0 ? GT : (int)blockDim.x, nw = nthr >> 5;  // (the generic evaluator picks its CTA size at launch)
-    eval_smem_layout(ge, f.nblk, d.L, d.nb, d.nat, ga.nu, nw, NAT == 0, &es, smem_raw);
+    eval_smem_layout(ge, f.nblk, d.L, d.nb, d.nat, ga.nu, nw, NAT == 0, MIX, &es, smem_raw);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nb = d.nb;
     const int NU = ga.nu;
     const int64_t gl = blockIdx.x / tiles_per_group;
@@ -569,8 +573,13 @@ __global__ void __launch_bounds__(NAT > 0 ? GT : GEN_WMAX * 32, NAT > 0 ? FP_EVA
         double2 p = d.ph1d[i];
         if (G.s2 < 0) p.y = -p.y;
         es.ph[i] = p;
+        if (MIX) es.phf[i] = make_float2((float)p.x, (float)p.y);
     }
     __syncthreads();
+    if (MIX) {                                                        // (after the barrier: Mhat is complete)
+        for (int i = threadIdx.x; i < nrt * nm9; i += nthr) es.Mf[i] = make_float2((float)es.M[i].x, (float)es.M[i].y);
+        __syncthreads();
+    }
 
     // ---- row by row, 64-process chunks: chunk c of a row goes to warp (c + rotation of the row) mod GW -- a static deal
     //      that depends on nothing but the row itself, so a row's sums do not depend on how rows were grouped or chunked
@@ -606,10 +615,20 @@ __global__ void __launch_bounds__(NAT > 0 ? GT : GEN_WMAX * 32, NAT > 0 ? FP_EVA
             const double2 *eB1 = d.evecc + ((size_t)(e1.y >> 6) * nb + (e1.y & 63u)) * nb;
             const int3 xc0 = unpack_qc(__ldg(d.qc + qx0)), xc1 = unpack_qc(__ldg(d.qc + qx1));
             double2 V0, V1;
-            if constexpr (NAT > 0) {
+            if constexpr (NAT > 0 && MIX) {
+                constexpr int NC = 3 * NAT;
+                float2 A0[NC], B0[NC], A1[NC], B1[NC];
+                const float2 *tA = G.s2 > 0 ? d.evec32 : d.evecc32;
+                const float2 *fA0 = tA + (eA0 - tabA), *fA1 = tA + (eA1 - tabA), *fB0 = d.evecc32 + (eB0 - d.evecc), *fB1 = d.evecc32 + (eB1 - d.evecc);
+#pragma unroll
+                for (int c = 0; c < NC; c++) { A0[c] = __ldg(fA0 + c); B0[c] = __ldg(fB0 + c); A1[c] = __ldg(fA1 + c); B1[c] = __ldg(fB1 + c); }
+                float2 W0, W1;
+                contract_process2_f32<NAT>(d, bs, es.Mf + rt * nm9, es.phf, A0, B0, premul(d, xc0), A1, B1, premul(d, xc1), W0, W1);
+                V0 = make_double2((double)W0.x, (double)W0.y); V1 = make_double2((double)W1.x, (double)W1.y);
+            } else if constexpr (NAT > 0) {
                 double2 A0[3 * (NAT > 0 ? NAT : 1)], B0[3 * (NAT > 0 ? NAT : 1)], A1[3 * (NAT > 0 ? NAT : 1)], B1[3 * (NAT > 0 ? NAT : 1)];
                 load_evec<3 * NAT>(eA0, A0); load_evec<3 * NAT>(eB0, B0); load_evec<3 * NAT>(eA1, A1); load_evec<3 * NAT>(eB1, B1);
-                contract_process2<NAT, PH8>(d, bs, A0, B0, premul(d, xc0), A1, B1, premul(d, xc1), V0, V1);
+                contract_process2<NAT, false>(d, bs, A0, B0, premul(d, xc0), A1, B1, premul(d, xc1), V0, V1);
             } else {
                 double2 *As = es.As + (size_t)warp * nb * 64 + lane;   // this lane's two leg-A vectors, [component][process]
                 if ((nb & 1) == 0) {
@@ -681,39 +700,39 @@ cudaError_t launch_enum_g(int order, const FpDev &d, const GroupArgs &ga, int64_
 static int eval_warps(const FpDev &d, const IfcDev &f, int ge) {
     if (d.nat <= 2) return GW;
     int nw = GEN_WMAX;
-    while (nw > 1 && eval_smem_layout(ge, f.nblk, d.L, d.nb, d.nat, enum_units(d), nw, true, nullptr, nullptr) > 226 * 1024) nw--;
+    while (nw > 1 && eval_smem_layout(ge, f.nblk, d.L, d.nb, d.nat, enum_units(d), nw, true, false, nullptr, nullptr) > 226 * 1024) nw--;
     return nw;
 }
-size_t eval_smem_bytes(const FpDev &d, const IfcDev &f, int ge) {
-    return eval_smem_layout(ge, f.nblk, d.L, d.nb, d.nat, enum_units(d), eval_warps(d, f, ge), d.nat > 2, nullptr, nullptr);
+size_t eval_smem_bytes(const FpDev &d, const IfcDev &f, int ge) {              // (with the FP32 copies of the mixed mode)
+    return eval_smem_layout(ge, f.nblk, d.L, d.nb, d.nat, enum_units(d), eval_warps(d, f, ge), d.nat > 2, d.nat <= 2, nullptr, nullptr);
 }
 
-template <int ORDER, int NAT>
+template <int ORDER, int NAT, bool MIX>
 static cudaError_t launch_eval_t(const FpDev &d, const IfcDev &f, const GroupArgs &ga, int64_t ngc, const double2 *pre,
                                  int64_t capw, const ListEnt *lists, const uint32_t *wcnt, int ge, double2 *partial,
                                  uint32_t *counts, cudaStream_t st) {
-    const size_t smem = eval_smem_bytes(d, f, ge);
+    const size_t smem = eval_smem_layout(ge, f.nblk, d.L, d.nb, d.nat, enum_units(d), eval_warps(d, f, ge), NAT == 0, MIX, nullptr, nullptr);
     const int tiles = (ga.rmaxg + ge - 1) / ge;
     const unsigned nthr = 32u * (unsigned)eval_warps(d, f, ge);
     static SmemGrant granted;
-    cudaError_t e = opt_in_smem(k_eval_g<ORDER, NAT, false>, smem, granted);
+    cudaError_t e = opt_in_smem(k_eval_g<ORDER, NAT, MIX>, smem, granted);
     if (e != cudaSuccess) return e;
-    k_eval_g<ORDER, NAT, false><<<(unsigned)(ngc * tiles), nthr, smem, st>>>(d, f, ga, pre, capw, lists, wcnt, ge, tiles, partial, counts);
+    k_eval_g<ORDER, NAT, MIX><<<(unsigned)(ngc * tiles), nthr, smem, st>>>(d, f, ga, pre, capw, lists, wcnt, ge, tiles, partial, counts);
     return cudaGetLastError();
 }
 
 cudaError_t launch_eval_g(int order, const FpDev &d, const IfcDev &f, const GroupArgs &ga, int64_t ngc, const double2 *pre,
                           int64_t capw, const ListEnt *lists, const uint32_t *wcnt, int ge, double2 *partial,
-                          uint32_t *counts, cudaStream_t st) {
+                          uint32_t *counts, bool mixed, cudaStream_t st) {
     if (ngc <= 0) return cudaSuccess;
 #define FP_ARGS d, f, ga, ngc, pre, capw, lists, wcnt, ge, partial, counts, st
     if (order == 3) {
-        if (d.nat == 1) return launch_eval_t<3, 1>(FP_ARGS);
-        if (d.nat == 2) return launch_eval_t<3, 2>(FP_ARGS);
-        return launch_eval_t<3, 0>(FP_ARGS);
+        if (d.nat == 1) return mixed ? launch_eval_t<3, 1, true>(FP_ARGS) : launch_eval_t<3, 1, false>(FP_ARGS);
+        if (d.nat == 2) return mixed ? launch_eval_t<3, 2, true>(FP_ARGS) : launch_eval_t<3, 2, false>(FP_ARGS);
+        return launch_eval_t<3, 0, false>(FP_ARGS);
     }
-    if (d.nat == 1) return launch_eval_t<4, 1>(FP_ARGS);
-    if (d.nat == 2) return launch_eval_t<4, 2>(FP_ARGS);
-    return launch_eval_t<4, 0>(FP_ARGS);
+    if (d.nat == 1) return mixed ? launch_eval_t<4, 1, true>(FP_ARGS) : launch_eval_t<4, 1, false>(FP_ARGS);
+    if (d.nat == 2) return mixed ? launch_eval_t<4, 2, true>(FP_ARGS) : launch_eval_t<4, 2, false>(FP_ARGS);
+    return launch_eval_t<4, 0, false>(FP_ARGS);
 #undef FP_ARGS
 }

@@ -185,7 +185,7 @@ size_t ifc_resident_bytes(int64_t n, int order, int nat) {
 
 size_t tables_resident_bytes(int nat, const int32_t mesh[3], long L) {
     size_t N = (size_t)mesh[0] * mesh[1] * mesh[2], nb = 3 * (size_t)nat, M = N * nb;
-    return align_up(M * sizeof(ModeRec)) + align_up(M * 16) * 2 + align_up(M * 8) * 2 + align_up(M * nb * 16) * 2 +
+    return align_up(M * sizeof(ModeRec)) + align_up(M * 16) * 2 + align_up(M * 8) * 2 + align_up(M * nb * 16) * 2 + align_up(M * nb * 8) * 2 +
            align_up((size_t)L * 16) + align_up(N * 4) + align_up(N * 8) + align_up(nat * 8) + 256 * 12;
 }
 
@@ -343,14 +343,15 @@ int fp_setup(const fp_crystal *crystal, const double *masses, const double *omeg
     double2 *aux = bump.take<double2>(M);
     double2 *evec = bump.take<double2>(M * nb);
     double2 *evecc = bump.take<double2>(M * nb);
+    float2 *evec32 = bump.take<float2>(M * nb), *evecc32 = bump.take<float2>(M * nb);
     double2 *ph1d = bump.take<double2>(L);
     int *qc = bump.take<int>(N);
     float2 *qmm = bump.take<float2>(N);
     double *masses_dev = bump.take<double>(nat);
-    if (!rec || !recf || !recn || !maxima || !occ || !aux || !evec || !evecc || !ph1d || !qc || !qmm || !masses_dev) {
+    if (!rec || !recf || !recn || !maxima || !occ || !aux || !evec || !evecc || !evec32 || !evecc32 || !ph1d || !qc || !qmm || !masses_dev) {
         fail(ctx, FP_ENOMEM, "workspace too small for the mode tables"); return bail(FP_ENOMEM);
     }
-    d.rec = rec; d.recf = recf; d.recn = recn; d.occ = occ; d.aux = aux; d.evec = evec; d.evecc = evecc; d.ph1d = ph1d; d.qc = qc; d.qmm = qmm;
+    d.rec = rec; d.recf = recf; d.recn = recn; d.occ = occ; d.aux = aux; d.evec = evec; d.evecc = evecc; d.evec32 = evec32; d.evecc32 = evecc32; d.ph1d = ph1d; d.qc = qc; d.qmm = qmm;
     // executed FP64 flops per matrix element: 13 complex MACs per block (nat <= 2: contract_process2); generic
     // atom count (contract_process2_staged): 12 per block + 3 per atom B that has blocks; 8 flop per complex MAC
     auto flops_elem = [&](const IfcHost &h) {
@@ -758,7 +759,7 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
                     CU(cudaStreamWaitEvent(st, ctx->ev_enum[b], 0));
                 }
                 { ProfScope p(ctx, CAT_RATES, st);
-                  CU(launch_eval_g(order, d, f, gc, n, pre, capw, lists[b], wcnt[b], ge_t, partial, cnt, st)); }
+                  CU(launch_eval_g(order, d, f, gc, n, pre, capw, lists[b], wcnt[b], ge_t, partial, cnt, ctx->precision == FP_PREC_MIXED, st)); }
                 if (overlap) CU(cudaEventRecord(ctx->ev_eval[b], st));
             }
             unsigned long long novf = 0;
@@ -923,6 +924,13 @@ int fp_set_symmetry(fp_ctx *ctx, int on) { if (!ctx) return FP_EINVAL; ctx->use_
 int fp_get_symmetry(const fp_ctx *ctx) {
     return ctx ? ((ctx->use_sym && ctx->sym23 ? 1 : 0) | (ctx->use_sym && ctx->sym34 ? 2 : 0)) : FP_EINVAL;
 }
+
+int fp_set_precision(fp_ctx *ctx, int mode) {
+    if (!ctx || (mode != FP_PREC_FP64 && mode != FP_PREC_MIXED)) return ctx ? fail(ctx, FP_EINVAL, "unknown precision mode") : FP_EINVAL;
+    ctx->precision = mode;
+    return FP_OK;
+}
+int fp_get_precision(const fp_ctx *ctx) { return ctx ? ctx->precision : FP_EINVAL; }
 
 int fp_set_target_symmetry(fp_ctx *ctx, int on) { if (!ctx) return FP_EINVAL; ctx->use_trs = on != 0; return FP_OK; }
 int fp_get_target_symmetry(const fp_ctx *ctx) { return ctx ? (ctx->use_trs && ctx->trs_ok ? 1 : 0) : FP_EINVAL; }

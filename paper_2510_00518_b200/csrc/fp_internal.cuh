@@ -38,6 +38,7 @@ struct FpDev {
     const double *occ;            // N*nb  f_lambda = 1/expm1(hbar omega/kB T)
     const double2 *evec;          // N*nb*nb mass-scaled eigenvectors e~ = e/sqrt(m)
     const double2 *evecc;         // N*nb*nb conj(e~): the conjugations of step 6 are table choices, not arithmetic
+    const float2 *evec32, *evecc32;   // the same rounded to FP32 (mixed-precision evaluator, fp_set_precision)
     const double2 *ph1d;          // L
     const int *qc;                // N packed mesh coordinates i1 | i2<<10 | i3<<20   (N_mu <= 1024)
     const float2 *qmm;            // N  {min, max} of the non-zero frequencies of a q-point, rounded outward to FP32
@@ -110,6 +111,7 @@ struct fp_ctx {
     int path = FP_PATH_AUTO;      // fp_set_path
     bool sym34 = false, sym23 = false;   // IFC4 / IFC3 is symmetric under the exchange of its last two legs (fp_setup)
     bool use_sym = true;          // fp_set_symmetry
+    int precision = FP_PREC_FP64; // fp_set_precision
     // time reversal (fp_set_target_symmetry): the mode arrays satisfy omega(-q,j) = omega(q,j), v(-q,j) = -v(q,j),
     // e(-q,j) = conj(e(q,j)) bit for bit (checked by fp_setup), so targets (q,j) and (-q,j) have the same rates and the
     // driver evaluates one of each pair (targets only in the irreducible part, N_list)
@@ -153,9 +155,10 @@ size_t eval_smem_bytes(const FpDev &d, const IfcDev &f, int ge);   // dynamic sh
 // work: a device counter the launcher zeroes (the units are dealt to the warps of a persistent grid)
 cudaError_t launch_enum_g(int order, const FpDev &d, const GroupArgs &ga, int64_t ngc, int64_t capw, ListEnt *lists,
                           uint32_t *wcnt, unsigned int *work, int sm_count, cudaStream_t st);
+// mixed: level-2 contraction in FP32 (nat <= 2 only; the generic evaluator stays FP64)
 cudaError_t launch_eval_g(int order, const FpDev &d, const IfcDev &f, const GroupArgs &ga, int64_t ngc, const double2 *pre,
                           int64_t capw, const ListEnt *lists, const uint32_t *wcnt, int ge, double2 *partial,
-                          uint32_t *counts, cudaStream_t st);
+                          uint32_t *counts, bool mixed, cudaStream_t st);
 void launch_finalize(int order, const FpDev &d, int64_t nt, int64_t rows_per_unit, const double2 *partial,
                      const uint32_t *counts, double c_over_n, double *gamma, double *wp, int64_t *cnt, cudaStream_t st);
 void launch_kappa(const FpDev &d, const double *gamma_total, double pref, double *kappa, cudaStream_t st);

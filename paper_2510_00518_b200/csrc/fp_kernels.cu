@@ -50,6 +50,8 @@ __global__ void k_tables(FpDev d, const double *omega, const double *eig, const 
         const double2 e = make_double2(eig[2 * c] / sm, eig[2 * c + 1] / sm);
         evec[c] = e;
         evecc[c] = make_double2(e.x, -e.y);
+        const_cast<float2 *>(d.evec32)[c] = make_float2((float)e.x, (float)e.y);
+        const_cast<float2 *>(d.evecc32)[c] = make_float2((float)e.x, -(float)e.y);
     }
     for (int64_t k = gid; k < d.L; k += stride) {                   // a4: phi = exp(2 pi i k / L)
         double s, c;

@@ -517,3 +517,29 @@ def test_per_process_terms(fp):
                 for i in rng.choice(len(g), size=min(3, len(g)), replace=False):
                     ref = bf.term4_dense(inp, lam, ch, triples[i])
                     assert abs(g[i] - ref) <= 1e-8 * abs(ref) + 1e-14 * np.abs(og).max(), (lam, ch, triples[i], g[i], ref)
+
+
+def test_mixed_precision_mode(fp):
+    """fp_set_precision(FP_PREC_MIXED): the level-2 contraction in FP32.  Counts and
+    the weighted phase space must not change at all (the decision and the weights stay FP64); Gamma carries the FP32
+    rounding of |V|^2 -- checked against the oracle at 2e-5 relative to the channel's largest rate, and it must really
+    differ from the FP64 result (the switch does something).  Off by default."""
+    inp = fp_inputs.make_tiny("diamond", mesh=(4, 4, 4))
+    t = np.ascontiguousarray(inp.targets4[12:36])
+    og, ow, oc = _oracle(inp).rates4(t, 3, 12)
+    og3, ow3, oc3 = _oracle(inp).rates3(inp.targets3)
+    with fp.Context.from_inputs(inp, scratch_bytes=256 << 20) as ctx:
+        assert ctx.get_precision() == fp.FP_PREC_FP64
+        g64, w64, c64 = ctx.rates4(t, 3, 12)
+        ctx.set_precision(fp.FP_PREC_MIXED)
+        assert ctx.get_precision() == fp.FP_PREC_MIXED
+        g, w, c = ctx.rates4(t, 3, 12)
+        g3, w3, c3 = ctx.rates3(inp.targets3)
+    assert np.array_equal(c, oc) and np.array_equal(w, w64) and np.array_equal(c3, oc3)
+    assert_rates_close(w3, ow3, "WP3 (mixed)")
+    for a, ref, what in ((g, og, "Gamma4"), (g3, og3, "Gamma3")):
+        scale = np.abs(ref).max(axis=0, keepdims=True)
+        err = np.abs(a - ref) / scale
+        assert err.max() < 2e-5, (what, err.max())
+    assert np.abs(g - g64).max() > 0.0
+    assert_rates_close(g64, og, "Gamma4 (FP64)")
