@@ -334,19 +334,22 @@ def main():
     tr = ncu_traffic(args.config, "k_eval_g" if split else "k_rates")
     dmma = fp.fp_probe_dmma_tflops()
     step_flops_rate = flops / (ms_step * 1e-3) / 1e12
+    mixed = args.precision == "mixed"                                       # FP32 FFMA pipe: 128 lanes/clk/SM, twice the FP64 rate
+    peak = FP64_PEAK_TFLOPS * (2.0 if mixed else 1.0)
     roofline = {"bound": "alu", "kernel": kname, "achieved": achieved,
-                "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_TFLOPS,
+                "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                 "traffic": tr["bytes"] if tr else None,
                 "traffic_source": ({"file": "profiles/ncu_traffic.json", "capture": tr["capture"], "launch": tr["launch"],
                                     "launch_ms": tr["duration_ms"], "list_bytes_of_that_launch": tr["list_bytes"]}
                                    if tr else None),
                 "algorithmic_bytes_per_launch_avg": 16.0 * evaluated / max(n_c, 1) if split else 20.0 * rows / max(n_c, 1),
-                "whole_step": {"achieved": step_flops_rate, "frac": step_flops_rate / FP64_PEAK_TFLOPS,
+                "whole_step": {"achieved": step_flops_rate, "frac": step_flops_rate / peak,
                                "what": "the same executed-flop model over the whole device-timed step (enumerator, "
                                        "pre-contraction and reduction included in the time, not in the flops)"},
                 "probes_tflops": {"dfma": probe, "dmma_m8n8k4": dmma["dmma"], "dfma_same_shape": dmma["dfma"],
                                   "dmma_and_dfma_interleaved": dmma["dmma_and_dfma"]},
-                "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (MEASURED_PEAKS.json has no FP64 "
+                "peak_source": ("FP32 (mixed mode): 148 SM x 128 FFMA/clk x 2 x 1.965 GHz; " if mixed else "") +
+                               "derived: 148 SM x 64 FP64 FMA/clk x 2 x 1.965 GHz (MEASURED_PEAKS.json has no FP64 "
                                f"entry); DFMA probe on this GPU measured {probe:.2f} TFLOP/s",
                 "flops_model": "matrix elements evaluated x executed flops of the level-2 contraction (nat <= 2: nblk x 13 complex "
                                "MAC x 8 flop; generic atom count: (12 nblk + 3 atoms) x 8; DESIGN.md §6); enumeration, decision "
