@@ -62,7 +62,6 @@ struct Bump {
         off = o + b;
         return reinterpret_cast<T *>(base + o);
     }
-    size_t left() const { size_t o = align_up(off); return o < end ? end - o : 0; }
 };
 
 int imod(long a, int n) { long r = a % n; return (int)(r < 0 ? r + n : r); }

@@ -74,8 +74,6 @@ __global__ void __launch_bounds__(256) k_pre4(FpDev d, IfcDev f, const int32_t *
 constexpr int RATES_MINB = 4;                 // k_rates: 128 registers
 constexpr int RT = 128;                       // threads per row CTA
 constexpr int RW = RT / 32;                   // warps
-constexpr int EVT = 128;                      // threads of a k_eval CTA (measured on B200, config 3: 32 -> 1363 ms, 64 -> 1232,
-                                              // 128 -> 1138, 256 -> 1425 per step: the row set-up wants several warps)
 constexpr int PCAP = 32 + 32 * 36;            // pending queue: < 32 left over + one 6x6 sub-tile of 32 q-points
 constexpr int QCAP = 64;                      // evaluation queue: < 32 left over + one stage-2 round
 
