@@ -14,7 +14,6 @@ struct BlkSmem {
     int4 *meta;        // nblk     {atomA | atomB<<16, d1, d2, d3}
     double2 *ph;       // L
     int *seg;          // nat*nat+1
-    unsigned *npk;     // nblk     d1 | d2 << 8 | d3 << 16 (meshes with L <= 256: the phase index is one dp4a)
 };
 
 // One block: u = sum_y (sum_x M[x][y] A[x]) Bc[y];  V += u * phase          (13 complex MAC = 52 DFMA)
@@ -74,37 +73,28 @@ __device__ __forceinline__ double2 contract_process(const FpDev &d, const BlkSme
 
 
 // Two processes per lane against one pass over the row's blocks: every Mhat_b read from shared memory feeds 2 x 13
-// complex MACs, and the two dependency chains interleave (NAT > 0 only).
-// PH8: L <= 256, so q (premultiplied) and the block's cell offset are packed bytes and the phase index is one dp4a.
-#ifndef FP_CONTRACT_V
-#define FP_CONTRACT_V 1
-#endif
-template <int NAT, bool PH8>
-__device__ __forceinline__ void contract_process2(const FpDev &d, const BlkSmem &bs, const double2 *A0, const double2 *B0,
-                                                  int3 q0, const double2 *A1, const double2 *B1, int3 q1, double2 &V0,
+// complex MACs, and the two dependency chains interleave (NAT > 0 only).  The conj(e~_B) vectors of both processes are
+// resident (B0, B1); the three leg-A components of an atom are loaded when that atom's blocks start (72 instead of 96
+// registers of eigenvector state: at the 168-register cap of three CTAs per SM the compiler otherwise serialises
+// independent DFMA chains -- measured 676 -> 644 ms per config-3 step).  Block order as everywhere else:
+// (atomA, atomB, dR).
+template <int NAT>
+__device__ __forceinline__ void contract_process2(const FpDev &d, const BlkSmem &bs, const double2 *__restrict__ eA0, const double2 *B0,
+                                                  int3 q0, const double2 *__restrict__ eA1, const double2 *B1, int3 q1, double2 &V0,
                                                   double2 &V1) {
     V0 = make_double2(0.0, 0.0); V1 = make_double2(0.0, 0.0);
-    const unsigned q0p = (unsigned)q0.x | ((unsigned)q0.y << 8) | ((unsigned)q0.z << 16);
-    const unsigned q1p = (unsigned)q1.x | ((unsigned)q1.y << 8) | ((unsigned)q1.z << 16);
 #pragma unroll
-    for (int a = 0; a < NAT; a++)
+    for (int a = 0; a < NAT; a++) {
+        double2 A0[3], A1[3];
+#pragma unroll
+        for (int x = 0; x < 3; x++) { A0[x] = __ldg(eA0 + 3 * a + x); A1[x] = __ldg(eA1 + 3 * a + x); }
 #pragma unroll
         for (int c = 0; c < NAT; c++) {
             const int b1 = bs.seg[a * NAT + c + 1];
             for (int b = bs.seg[a * NAT + c]; b < b1; b++) {
-                int i0, i1;
-                if (PH8) {
-                    const unsigned n = bs.npk[b];
-                    const unsigned x0 = __dp4a(q0p, n, 0u), x1 = __dp4a(q1p, n, 0u);
-                    i0 = d.Lmask >= 0 ? (int)(x0 & (unsigned)d.Lmask) : (int)(x0 % (unsigned)d.L);
-                    i1 = d.Lmask >= 0 ? (int)(x1 & (unsigned)d.Lmask) : (int)(x1 % (unsigned)d.L);
-                } else {
-                    const int4 m = bs.meta[b];
-                    i0 = phase_idx(d, q0, m.y, m.z, m.w); i1 = phase_idx(d, q1, m.y, m.z, m.w);
-                }
-                const double2 p0 = bs.ph[i0], p1 = bs.ph[i1];
+                const int4 m = bs.meta[b];
+                const double2 p0 = bs.ph[phase_idx(d, q0, m.y, m.z, m.w)], p1 = bs.ph[phase_idx(d, q1, m.y, m.z, m.w)];
                 const double2 *M = bs.M + 9 * b;
-#if FP_CONTRACT_V == 1
                 double2 u0 = make_double2(0.0, 0.0), u1 = make_double2(0.0, 0.0);
 #pragma unroll
                 for (int y = 0; y < 3; y++) {
@@ -112,40 +102,14 @@ __device__ __forceinline__ void contract_process2(const FpDev &d, const BlkSmem 
 #pragma unroll
                     for (int x = 0; x < 3; x++) {
                         const double2 mm = M[3 * x + y];
-                        cfma(t0, mm, A0[3 * a + x]); cfma(t1, mm, A1[3 * a + x]);
+                        cfma(t0, mm, A0[x]); cfma(t1, mm, A1[x]);
                     }
                     cfma(u0, t0, B0[3 * c + y]); cfma(u1, t1, B1[3 * c + y]);
                 }
                 cfma(V0, u0, p0); cfma(V1, u1, p1);
-#else
-                // t[y] = sum_x M[x][y] A[x]: twelve independent chains (2 processes x 3 columns x re/im), row by row of M
-                double2 t0[3], t1[3];
-#pragma unroll
-                for (int y = 0; y < 3; y++) { t0[y] = make_double2(0.0, 0.0); t1[y] = make_double2(0.0, 0.0); }
-#pragma unroll
-                for (int x = 0; x < 3; x++) {
-                    const double2 a0 = A0[3 * a + x], a1 = A1[3 * a + x];
-                    double2 mm[3];
-#pragma unroll
-                    for (int y = 0; y < 3; y++) mm[y] = M[3 * x + y];
-#pragma unroll
-                    for (int y = 0; y < 3; y++) { t0[y].x = fma(mm[y].x, a0.x, t0[y].x); t1[y].x = fma(mm[y].x, a1.x, t1[y].x); }
-#pragma unroll
-                    for (int y = 0; y < 3; y++) { t0[y].y = fma(mm[y].x, a0.y, t0[y].y); t1[y].y = fma(mm[y].x, a1.y, t1[y].y); }
-#pragma unroll
-                    for (int y = 0; y < 3; y++) { t0[y].x = fma(-mm[y].y, a0.y, t0[y].x); t1[y].x = fma(-mm[y].y, a1.y, t1[y].x); }
-#pragma unroll
-                    for (int y = 0; y < 3; y++) { t0[y].y = fma(mm[y].y, a0.x, t0[y].y); t1[y].y = fma(mm[y].y, a1.x, t1[y].y); }
-                }
-                // u = sum_y t[y] Bc[y] as two partial sums per process, then V += u phase
-                double2 ua0 = make_double2(0.0, 0.0), ub0 = make_double2(0.0, 0.0), ua1 = make_double2(0.0, 0.0), ub1 = make_double2(0.0, 0.0);
-                cfma(ua0, t0[0], B0[3 * c]); cfma(ub0, t0[1], B0[3 * c + 1]); cfma(ua1, t1[0], B1[3 * c]); cfma(ub1, t1[1], B1[3 * c + 1]);
-                cfma(ua0, t0[2], B0[3 * c + 2]); cfma(ua1, t1[2], B1[3 * c + 2]);
-                const double2 u0 = make_double2(ua0.x + ub0.x, ua0.y + ub0.y), u1 = make_double2(ua1.x + ub1.x, ua1.y + ub1.y);
-                cfma(V0, u0, p0); cfma(V1, u1, p1);
-#endif
             }
         }
+    }
 }
 
 // Mixed precision (fp_set_precision): the same two-process contraction in FP32 -- Mhat, phases and both

@@ -398,7 +398,6 @@ struct EvalSmem {
     double2 *ph;       // L
     double2 *e1;       // ge * nb        level-1 eigenvectors (4ph)
     int4 *meta;        // nblk
-    unsigned *npk;     // nblk           packed cell offsets of the blocks (BlkSmem::npk)
     int *seg;          // nat*nat+1 (padded to 4)
     unsigned *rpre;    // ge * (NU + 1)  prefix sums of the NU slot lengths of a row: its slots read as one list
     double *rowfac;    // ge             row factors of the weight: occ_row / (omega [omega'])
@@ -417,7 +416,6 @@ __host__ __device__ inline size_t eval_smem_layout(int ge, int nblk, int L, int 
     auto take = [&](size_t bytes) { size_t r = o; o += (bytes + 15) & ~(size_t)15; return r; };
     const size_t oM = take((size_t)ge * nblk * 9 * sizeof(double2)), oph = take((size_t)L * sizeof(double2)),
                  oe1 = take((size_t)ge * nb * sizeof(double2)), ometa = take((size_t)nblk * sizeof(int4)),
-                 onpk = take((size_t)nblk * sizeof(unsigned)),
                  oseg = take((size_t)(nat * nat + 1) * sizeof(int)), orowp = take((size_t)ge * (NU + 1) * sizeof(unsigned)),
                  orf = take((size_t)ge * sizeof(double)), oro = take((size_t)ge * sizeof(long long)),
                  och = take((size_t)(ge + 1) * sizeof(int)), oaG = take((size_t)nw * ge * sizeof(double)),
@@ -427,7 +425,7 @@ __host__ __device__ inline size_t eval_smem_layout(int ge, int nblk, int L, int 
     if (es) {
         es->M = reinterpret_cast<double2 *>(base + oM); es->ph = reinterpret_cast<double2 *>(base + oph);
         es->e1 = reinterpret_cast<double2 *>(base + oe1); es->meta = reinterpret_cast<int4 *>(base + ometa);
-        es->seg = reinterpret_cast<int *>(base + oseg); es->npk = reinterpret_cast<unsigned *>(base + onpk); es->rpre = reinterpret_cast<unsigned *>(base + orowp);
+        es->seg = reinterpret_cast<int *>(base + oseg); es->rpre = reinterpret_cast<unsigned *>(base + orowp);
         es->rowfac = reinterpret_cast<double *>(base + orf); es->rold = reinterpret_cast<long long *>(base + oro);
         es->chunk0 = reinterpret_cast<int *>(base + och); es->accG = reinterpret_cast<double *>(base + oaG);
         es->accW = reinterpret_cast<double *>(base + oaW); es->accC = reinterpret_cast<unsigned *>(base + oaC);
@@ -507,7 +505,6 @@ __global__ void __launch_bounds__(NAT > 0 ? GT : GEN_WMAX * 32, NAT > 0 ? (MIX ?
     for (int i = threadIdx.x; i < f.nblk; i += nthr) {
         const int4 m = f.blk_meta[i];
         es.meta[i] = m;
-        es.npk[i] = (unsigned)m.y | ((unsigned)m.z << 8) | ((unsigned)m.w << 16);
     }
     for (int i = threadIdx.x; i <= d.nat * d.nat; i += nthr) es.seg[i] = f.seg[i];
     if (ORDER == 3) {
@@ -584,7 +581,7 @@ __global__ void __launch_bounds__(NAT > 0 ? GT : GEN_WMAX * 32, NAT > 0 ? (MIX ?
     // ---- row by row, 64-process chunks: chunk c of a row goes to warp (c + rotation of the row) mod GW -- a static deal
     //      that depends on nothing but the row itself, so a row's sums do not depend on how rows were grouped or chunked
     BlkSmem bs;
-    bs.meta = es.meta; bs.ph = es.ph; bs.seg = es.seg; bs.M = es.M; bs.npk = es.npk;
+    bs.meta = es.meta; bs.ph = es.ph; bs.seg = es.seg; bs.M = es.M;
     const double2 *tabA = G.s2 > 0 ? d.evec : d.evecc;
     for (int rt = 0; rt < nrt; rt++) {
         const unsigned *rp = es.rpre + rt * (NU + 1);
@@ -626,9 +623,9 @@ __global__ void __launch_bounds__(NAT > 0 ? GT : GEN_WMAX * 32, NAT > 0 ? (MIX ?
                 contract_process2_f32<NAT>(d, bs, es.Mf + rt * nm9, es.phf, A0, B0, premul(d, xc0), A1, B1, premul(d, xc1), W0, W1);
                 V0 = make_double2((double)W0.x, (double)W0.y); V1 = make_double2((double)W1.x, (double)W1.y);
             } else if constexpr (NAT > 0) {
-                double2 A0[3 * (NAT > 0 ? NAT : 1)], B0[3 * (NAT > 0 ? NAT : 1)], A1[3 * (NAT > 0 ? NAT : 1)], B1[3 * (NAT > 0 ? NAT : 1)];
-                load_evec<3 * NAT>(eA0, A0); load_evec<3 * NAT>(eB0, B0); load_evec<3 * NAT>(eA1, A1); load_evec<3 * NAT>(eB1, B1);
-                contract_process2<NAT, false>(d, bs, A0, B0, premul(d, xc0), A1, B1, premul(d, xc1), V0, V1);
+                double2 B0[3 * (NAT > 0 ? NAT : 1)], B1[3 * (NAT > 0 ? NAT : 1)];
+                load_evec<3 * NAT>(eB0, B0); load_evec<3 * NAT>(eB1, B1);
+                contract_process2<NAT>(d, bs, eA0, B0, premul(d, xc0), eA1, B1, premul(d, xc1), V0, V1);
             } else {
                 double2 *As = es.As + (size_t)warp * nb * 64 + lane;   // this lane's two leg-A vectors, [component][process]
                 if ((nb & 1) == 0) {
