@@ -76,7 +76,8 @@ __device__ __forceinline__ double2 contract_process(const FpDev &d, const BlkSme
 // complex MACs, and the two dependency chains interleave (NAT > 0 only).  The conj(e~_B) vectors of both processes are
 // resident (B0, B1); the three leg-A components of an atom are loaded when that atom's blocks start (72 instead of 96
 // registers of eigenvector state: at the 168-register cap of three CTAs per SM the compiler otherwise serialises
-// independent DFMA chains -- measured 676 -> 644 ms per config-3 step).  Block order as everywhere else:
+// independent DFMA chains -- measured 676 -> 651 ms per config-3 step, and 630 with the t-step written row by row of
+// Mhat).  Block order as everywhere else:
 // (atomA, atomB, dR).
 template <int NAT>
 __device__ __forceinline__ void contract_process2(const FpDev &d, const BlkSmem &bs, const double2 *__restrict__ eA0, const double2 *B0,
@@ -96,16 +97,18 @@ __device__ __forceinline__ void contract_process2(const FpDev &d, const BlkSmem 
                 const double2 p0 = bs.ph[phase_idx(d, q0, m.y, m.z, m.w)], p1 = bs.ph[phase_idx(d, q1, m.y, m.z, m.w)];
                 const double2 *M = bs.M + 9 * b;
                 double2 u0 = make_double2(0.0, 0.0), u1 = make_double2(0.0, 0.0);
+                double2 t0[3], t1[3];                                 // t[y] = sum_x Mhat[x][y] A[x], row by row of Mhat: the six
+#pragma unroll                                                        // t's of the two processes are twelve independent DFMA chains
+                for (int y = 0; y < 3; y++) { t0[y] = make_double2(0.0, 0.0); t1[y] = make_double2(0.0, 0.0); }
 #pragma unroll
-                for (int y = 0; y < 3; y++) {
-                    double2 t0 = make_double2(0.0, 0.0), t1 = make_double2(0.0, 0.0);
+                for (int x = 0; x < 3; x++)
 #pragma unroll
-                    for (int x = 0; x < 3; x++) {
+                    for (int y = 0; y < 3; y++) {
                         const double2 mm = M[3 * x + y];
-                        cfma(t0, mm, A0[x]); cfma(t1, mm, A1[x]);
+                        cfma(t0[y], mm, A0[x]); cfma(t1[y], mm, A1[x]);
                     }
-                    cfma(u0, t0, B0[3 * c + y]); cfma(u1, t1, B1[3 * c + y]);
-                }
+#pragma unroll
+                for (int y = 0; y < 3; y++) { cfma(u0, t0[y], B0[3 * c + y]); cfma(u1, t1[y], B1[3 * c + y]); }
                 cfma(V0, u0, p0); cfma(V1, u1, p1);
             }
         }
