@@ -32,7 +32,12 @@ __device__ __forceinline__ int q_index(const FpDev &d, int3 c) { return c.x + d.
 // index into ph1d of phi(q,R): qm = (i1 m1, i2 m2, i3 m3), n = cell offset reduced to [0,N_mu)
 __device__ __forceinline__ int phase_idx(const FpDev &d, int3 qm, int n1, int n2, int n3) {
     unsigned x = (unsigned)(qm.x * n1 + qm.y * n2 + qm.z * n3);
-    return d.Lmask >= 0 ? (int)(x & (unsigned)d.Lmask) : (int)(x % (unsigned)d.L);
+    if (d.Lmask >= 0) return (int)(x & (unsigned)d.Lmask);
+    // x mod L without a division: floor(x Lmagic / 2^32) with Lmagic = ceil(2^32 / L) is floor(x / L) or one more than
+    // that for every 32-bit x, so one conditional correction makes it exact
+    const unsigned q = __umulhi(x, d.Lmagic);
+    int r = (int)(x - q * (unsigned)d.L);
+    return r < 0 ? r + d.L : r;
 }
 __device__ __forceinline__ int3 premul(const FpDev &d, int3 c) { return make_int3(c.x * d.m1, c.y * d.m2, c.z * d.m3); }
 

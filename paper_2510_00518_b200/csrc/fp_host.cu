@@ -314,6 +314,7 @@ int fp_setup(const fp_crystal *crystal, const double *masses, const double *omeg
     d.nat = nat; d.nb = (int)nb; d.N = (int)N; d.N1 = mesh[0]; d.N2 = mesh[1]; d.N3 = mesh[2];
     d.L = (int)L; d.m1 = (int)(L / mesh[0]); d.m2 = (int)(L / mesh[1]); d.m3 = (int)(L / mesh[2]);
     d.Lmask = (L & (L - 1)) == 0 ? (int)(L - 1) : -1;
+    d.Lmagic = (unsigned)((((unsigned long long)1 << 32) + (unsigned long long)L - 1) / (unsigned long long)L);
     d.scale = br->scale; d.ncut = br->ncut; d.sigma_const = br->sigma_const; d.T = T;
     {   // B_mu = b_mu/N_mu, pinned order; host code is compiled with -ffp-contract=off
         const double *a1 = crystal->lattvec, *a2 = a1 + 3, *a3 = a1 + 6;

@@ -25,6 +25,7 @@ struct FpDev {
     int nat, nb, N, N1, N2, N3;
     int L, m1, m2, m3;            // L = lcm(N1,N2,N3); m_mu = L/N_mu ; phase(q,R) = ph1d[(sum_mu i_mu m_mu n_mu) mod L]
     int Lmask;                    // L-1 if L is a power of two, else -1
+    unsigned Lmagic;              // ceil(2^32 / L): x mod L by a multiply (phase_idx), L not a power of two
     double B[9];                  // B_mu = b_mu/N_mu, pinned arithmetic
     double scale, ncut, sigma_const, T;
     float pfK1, pfC2;             // FP32 pre-filter, stage 2: admit iff Delta_f^2 <= pfK1*|u_a-u_b|_f^2 + pfC2
