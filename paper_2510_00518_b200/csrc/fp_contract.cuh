@@ -155,8 +155,8 @@ __device__ __forceinline__ void contract_process2_f32(const FpDev &d, const BlkS
 
 // The same for any atom count, every eigenvector component fetched once: the leg-A vectors of the two processes are
 // staged by the caller in shared memory (As[comp * 64 + 32 h], already offset by the lane: each lane reads back only
-// what it wrote), the loop runs atom-B-major with the three conj(e~_B) components of atom c in registers (those of
-// atom c + 1 are fetched while c is computed), and the sum over y is taken once per atom c:
+// what it wrote), the loop runs atom-B-major with the three conj(e~_B) components of atom c in registers, and the sum
+// over y is taken once per atom c:
 //   W_c[y] = sum_{b : atomB_b = c} phi_b sum_x Mhat_b[x][y] A(atomA_b, x),   V = sum_c sum_y W_c[y] conj(e~_B(c, y))
 // -- 12 complex MACs per block and process plus 3 per atom c.  Blocks are sorted by (atomA, atomB): seg[a nat + c].
 __device__ __forceinline__ void contract_process2_staged(const FpDev &d, const BlkSmem &bs, const double2 *As,
@@ -164,19 +164,12 @@ __device__ __forceinline__ void contract_process2_staged(const FpDev &d, const B
                                                          const double2 *__restrict__ eB1, int3 q1, double2 &V0, double2 &V1) {
     V0 = make_double2(0.0, 0.0); V1 = make_double2(0.0, 0.0);
     const int nat = d.nat;
-    double2 Bn0[3], Bn1[3];
-#pragma unroll
-    for (int y = 0; y < 3; y++) { Bn0[y] = __ldg(eB0 + y); Bn1[y] = __ldg(eB1 + y); }
     for (int c = 0; c < nat; c++) {
         double2 B0[3], B1[3], W0[3], W1[3];
 #pragma unroll
         for (int y = 0; y < 3; y++) {
-            B0[y] = Bn0[y]; B1[y] = Bn1[y];
+            B0[y] = __ldg(eB0 + 3 * c + y); B1[y] = __ldg(eB1 + 3 * c + y);   // (first needed after all blocks of atom c)
             W0[y] = make_double2(0.0, 0.0); W1[y] = make_double2(0.0, 0.0);
-        }
-        if (c + 1 < nat) {
-#pragma unroll
-            for (int y = 0; y < 3; y++) { Bn0[y] = __ldg(eB0 + 3 * (c + 1) + y); Bn1[y] = __ldg(eB1 + 3 * (c + 1) + y); }
         }
         for (int a = 0; a < nat; a++) {
             const int b0 = bs.seg[a * nat + c], b1 = bs.seg[a * nat + c + 1];
@@ -184,6 +177,7 @@ __device__ __forceinline__ void contract_process2_staged(const FpDev &d, const B
             double2 A0[3], A1[3];
 #pragma unroll
             for (int x = 0; x < 3; x++) { A0[x] = As[(3 * a + x) * 64]; A1[x] = As[(3 * a + x) * 64 + 32]; }
+#pragma unroll 2                                                      // (measured on B200, config 4: 1 / 2 / 3 / 4 -> 3180 / 3091 / 3183 / 3208 ms)
             for (int b = b0; b < b1; b++) {
                 const int4 m = bs.meta[b];
                 const double2 p0 = bs.ph[phase_idx(d, q0, m.y, m.z, m.w)], p1 = bs.ph[phase_idx(d, q1, m.y, m.z, m.w)];
