@@ -32,7 +32,7 @@ constexpr int NUMAX = FP_ENUM_NU;             // enumeration units (shares of th
 constexpr int GT = GW * 32;
 constexpr int RMAX = FP_GROUP_RMAX;           // rows per enumerator group
 #ifndef FP_ENUM_QC
-#define FP_ENUM_QC 1024
+#define FP_ENUM_QC 2048         // measured (B200): 1024 / 1536 / 2048 / 2560 -> k_enum_g 249 / 244 / 243 / 298 ms at config 3 (2560 costs a CTA per SM), 504 / 479 / 457 / 452 ms at config 4
 #endif
 #ifndef FP_ENUM_MINB
 #define FP_ENUM_MINB 6
