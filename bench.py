@@ -329,7 +329,7 @@ def main():
     split = n_en > 0
     achieved = flops / (ms_c * 1e-3) / 1e12 if ms_c > 0 else 0.0
     probe = fp.fp_probe_fp64_tflops()
-    kname = ("k_eval (V3/V4 level-2 contraction + row sums over the process lists; the enumerator k_enum is timed "
+    kname = ("k_eval_g (V3/V4 level-2 contraction + row sums over the process lists; the enumerator k_enum_g is timed "
              "separately, see kernel_ms_per_step)") if split else "k_rates (fused enumerate + V3/V4 contraction + weights)"
     tr = ncu_traffic(args.config, "k_eval_g" if split else "k_rates")
     dmma = fp.fp_probe_dmma_tflops()

@@ -86,8 +86,8 @@ typedef struct {
 /* Device-time profile of the kernels launched since the last fp_profile_reset (CUDA events on the launch stream).   */
 typedef struct {
     double  ms_precontract, ms_rates, ms_reduce;      /* summed launch durations, ms: per-target pre-contraction, the  */
-    int64_t n_precontract, n_rates, n_reduce;         /* evaluator (k_eval; fused: k_rates), per-mode reduction; launches */
-    int64_t rows;           /* rows ((target, channel[, lambda']) units, one CTA each per kernel)                        */
+    int64_t n_precontract, n_rates, n_reduce;         /* evaluator (k_eval_g; fused: k_rates), per-mode reduction; launches */
+    int64_t rows;           /* rows ((target, channel[, lambda']) units of work: one process list and one partial sum each)  */
     int64_t candidates;     /* momentum-conserving candidates examined by the enumerator                            */
     int64_t prefiltered;    /* candidates admitted by the FP32 pre-filter (superset of the allowed ones)            */
     int64_t processes;      /* allowed processes (pinned FP64 decision) evaluated                                   */
@@ -100,7 +100,7 @@ typedef struct {
 
 /* Bytes of workspace fp_setup needs for its resident tables plus `scratch_bytes` of per-call scratch: per-target
  * pre-contracted tables, 20 bytes per row of partial sums and -- in half of it -- the process lists of the split path
- * (4 x N x nb^2 bytes per row; a larger scratch means more rows per launch: 48 GB gives 43,689 rows at 16x16x16, nb = 6;
+ * (4 x N x nb^2 bytes per row; a larger scratch means more rows per launch: 48 GB gives 43,668 rows at 16x16x16, nb = 6;
  * below 256 rows of lists the fused path runs instead, see fp_set_path).  ifc3/ifc4 may be NULL.  Returns 0 on invalid
  * arguments.                                                                                                          */
 size_t fp_workspace_bytes(const fp_crystal *crystal, const int32_t mesh[3], const fp_ifc *ifc3, const fp_ifc *ifc4,
