@@ -139,6 +139,18 @@ int fp_rates4(fp_ctx *ctx, const int32_t *targets, int64_t ntargets, int32_t qp_
  * modes with Gamma <= 0.   gamma_total loc N*nb (1/ps);  kappa loc 9 (row-major 3x3, W/(m K)).                      */
 int fp_kappa_rta(fp_ctx *ctx, const double *gamma_total, double *kappa, fp_memloc loc, void *stream);
 
+/* The same kappa for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc).  fp_kappa_rta_static calls no cudaMalloc / cudaFree and touches none of the context's workspace
+ * scratch: a multi-CTA reduction (fixed summation order, so it equals fp_kappa_rta to rounding order, not bit for bit)
+ * whose scratch -- the staged rates for FP_MEM_HOST, per-CTA partial sums, a ticket counter -- is ONE static device
+ * array of FP_NOALLOC_MAX_MODES doubles + 5 KB (529,040 bytes), held by every GPU that loads the library until the
+ * process exits.  Limit: N*nb <= FP_NOALLOC_MAX_MODES, else FP_EINVAL (fp_last_error names both numbers).  The device
+ * of fp_setup must be current (FP_ESTATE otherwise).  All calls share the array: calls that overlap on the GPU (two
+ * streams, two host threads, two contexts on one device) race on it; calls ordered on one stream do not.
+ * FP_MEM_HOST synchronises the stream before returning; FP_MEM_DEVICE is asynchronous.                                */
+#define FP_NOALLOC_MAX_MODES 65536
+int fp_kappa_rta_static(fp_ctx *ctx, const double *gamma_total, double *kappa, fp_memloc loc, void *stream);
+
 /* Debug export (not timed): the allowed-process list of one target and 3ph channel as (lambda', lambda'') pairs.
  *   pairs HOST cap*2 int32; *n receives the number of allowed processes (may exceed cap; only cap are written).
  * Order is the enumerator's (ascending q', j', j''); compare as sets.                                               */

@@ -20,15 +20,16 @@ FP_OK, FP_EINVAL, FP_ENOMEM, FP_ECUDA, FP_ESTATE = 0, -1, -2, -3, -4
 FP_PATH_AUTO, FP_PATH_FUSED, FP_PATH_SPLIT, FP_PATH_SPLIT_SERIAL = 0, 1, 2, 3
 FP_PREC_FP64, FP_PREC_MIXED = 0, 1
 FP_MEM_HOST, FP_MEM_DEVICE = 0, 1
+FP_NOALLOC_MAX_MODES = 65536     # include/fourphonon.h: largest N*nb fp_kappa_rta_static accepts
 
 _PKG = Path(__file__).resolve().parent
 _CSRC = _PKG / "csrc"
 _LIB = _PKG / "libfourphonon_b200.so"
-_SOURCES = ["fp_kernels.cu", "fp_rates.cu", "fp_group.cu", "fp_host.cu"]
+_SOURCES = ["fp_kernels.cu", "fp_rates.cu", "fp_group.cu", "fp_host.cu", "fp_noalloc.cu"]
 
 # every symbol include/fourphonon.h declares (tests check that the built library exports all of them)
 EXPORTED_SYMBOLS = [
-    "fp_workspace_bytes", "fp_setup", "fp_rates3", "fp_rates4", "fp_kappa_rta", "fp_list3", "fp_list4",
+    "fp_workspace_bytes", "fp_setup", "fp_rates3", "fp_rates4", "fp_kappa_rta", "fp_kappa_rta_static", "fp_list3", "fp_list4",
     "fp_terms3", "fp_terms4", "fp_set_path", "fp_set_symmetry", "fp_get_symmetry", "fp_set_target_symmetry", "fp_get_target_symmetry", "fp_set_precision", "fp_get_precision", "fp_set_prefilter", "fp_profile_enable", "fp_profile_reset", "fp_profile_get", "fp_probe_fp64_tflops", "fp_probe_dmma_tflops", "fp_constants",
     "fp_last_error", "fp_version", "fp_destroy",
 ]
@@ -127,6 +128,8 @@ def load_library():
     lib.fp_rates4.argtypes = [vp, vp, i64, i32, i32, vp, vp, vp, C.c_int, vp]
     lib.fp_kappa_rta.restype = C.c_int
     lib.fp_kappa_rta.argtypes = [vp, vp, vp, C.c_int, vp]
+    lib.fp_kappa_rta_static.restype = C.c_int
+    lib.fp_kappa_rta_static.argtypes = [vp, vp, vp, C.c_int, vp]
     lib.fp_list3.restype = C.c_int
     lib.fp_list3.argtypes = [vp, i32, i32, vp, i64, C.POINTER(i64), vp]
     lib.fp_list4.restype = C.c_int
@@ -374,6 +377,26 @@ class Context:
                     raise FourPhononError(FP_EINVAL, "gamma_total must have N*nb entries")
                 k = np.zeros((3, 3))
                 rc = self.lib.fp_kappa_rta(self.ctx, g.ctypes.data, k.ctypes.data, FP_MEM_HOST, _stream_ptr(stream))
+        self._check(rc)
+        return k
+
+    def kappa_rta_static(self, gamma_total, stream=None):
+        """fp_kappa_rta_static: kappa_rta without any allocation on the library side (static device scratch; N*nb <=
+        FP_NOALLOC_MAX_MODES; calls that overlap on the GPU race).  numpy in -> numpy out, torch CUDA in -> torch out."""
+        torch = self._torch
+        with torch.cuda.device(self.device):
+            if _is_torch(gamma_total):
+                g = gamma_total.contiguous().to(torch.float64).reshape(-1)
+                if g.numel() != self.nmodes:
+                    raise FourPhononError(FP_EINVAL, "gamma_total must have N*nb entries")
+                k = torch.empty((3, 3), dtype=torch.float64, device=g.device)
+                rc = self.lib.fp_kappa_rta_static(self.ctx, g.data_ptr(), k.data_ptr(), FP_MEM_DEVICE, _stream_ptr(stream))
+            else:
+                g = np.ascontiguousarray(gamma_total, dtype=np.float64).reshape(-1)
+                if g.size != self.nmodes:
+                    raise FourPhononError(FP_EINVAL, "gamma_total must have N*nb entries")
+                k = np.zeros((3, 3))
+                rc = self.lib.fp_kappa_rta_static(self.ctx, g.ctypes.data, k.ctypes.data, FP_MEM_HOST, _stream_ptr(stream))
         self._check(rc)
         return k
 
