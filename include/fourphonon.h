@@ -32,10 +32,11 @@
  * Limits
  *   natoms <= 21 (64-bit branch masks), N_mu <= 1024, N <= 2^20 q-points, lcm(N1,N2,N3) <= 4096 (phase table in shared
  *   memory).  The clusters of an IFC list are regrouped into contraction blocks (atomA, atomB, R_A - R_B mod mesh) of
- *   its last two legs; the per-row table of a list (144 bytes per block) lives in the shared memory of one SM, which
- *   caps a list at about 1,400 blocks (the synthetic configs have 10-152; first-principles silicon IFC3 sets within
- *   the usual cutoffs have a few hundred).  fp_rates3 / fp_rates4 return FP_ENOMEM beyond that and fp_last_error names
- *   the block count.
+ *   its last two legs; the per-row table of a list (144 bytes per block) normally lives in the shared memory of one SM,
+ *   which holds about 1,400 blocks (the synthetic configs have 10-152).  An IFC3 list beyond that is still served: its
+ *   table is per target, not per row, and the 3ph kernels then read it from global memory (slower per block; the
+ *   remaining cap, 16 bytes of block metadata per block in shared memory, is about 12,000 blocks).  An IFC4 list beyond
+ *   about 1,400 blocks is refused: fp_rates4 returns FP_ENOMEM and fp_last_error names the block count.
  *
  * Errors
  *   Every call returns FP_OK (0) or a negative code; nothing throws or aborts.  fp_last_error(ctx) (ctx may be NULL

@@ -410,11 +410,12 @@ struct EvalSmem {
     float2 *Mf, *phf;  // ge * nblk*9, L mixed precision: Mhat and the phases rounded to FP32
 };
 // nw = warps of the CTA; stage: the generic evaluator (NAT = 0) stages one eigenvector per process of every warp's chunk
+// mg: the Mhat tables stay in global memory (3ph, IFC3 lists too long for shared memory)
 __host__ __device__ inline size_t eval_smem_layout(int ge, int nblk, int L, int nb, int nat, int NU, int nw, bool stage, bool mixed,
-                                                   EvalSmem *es, unsigned char *base) {
+                                                   EvalSmem *es, unsigned char *base, bool mg = false) {
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t r = o; o += (bytes + 15) & ~(size_t)15; return r; };
-    const size_t oM = take((size_t)ge * nblk * 9 * sizeof(double2)), oph = take((size_t)L * sizeof(double2)),
+    const size_t oM = take(mg ? 0 : (size_t)ge * nblk * 9 * sizeof(double2)), oph = take((size_t)L * sizeof(double2)),
                  oe1 = take((size_t)ge * nb * sizeof(double2)), ometa = take((size_t)nblk * sizeof(int4)),
                  oseg = take((size_t)(nat * nat + 1) * sizeof(int)), orowp = take((size_t)ge * (NU + 1) * sizeof(unsigned)),
                  orf = take((size_t)ge * sizeof(double)), oro = take((size_t)ge * sizeof(long long)),
@@ -440,7 +441,8 @@ __host__ __device__ inline size_t eval_smem_layout(int ge, int nblk, int L, int 
 #endif
 constexpr int GEN_WMAX = 8;                   // warps of a generic-evaluator CTA, at most (as many as the staging leaves room for)
 // MIX: level-2 contraction in FP32 (fp_set_precision; NAT > 0 only)
-template <int ORDER, int NAT, bool MIX>
+// MG:  3ph only: Mhat of a row is read from the level-0 table in global memory, not from a shared-memory copy
+template <int ORDER, int NAT, bool MIX, bool MG = false>
 __global__ void __launch_bounds__(NAT > 0 ? GT : GEN_WMAX * 32, NAT > 0 ? (MIX ? 4 : FP_EVAL_MINB) : 1) k_eval_g(FpDev d, IfcDev f, GroupArgs ga, const double2 *pre, int64_t capw,
                                                   const ListEnt *lists, const uint32_t *wcnt, int ge, int tiles_per_group,
                                                   double2 *partial, uint32_t *counts) {
@@ -448,7 +450,8 @@ __global__ void __launch_bounds__(NAT > 0 ? GT : GEN_WMAX * 32, NAT > 0 ? (MIX ?
     __shared__ int s_nitems;
     EvalSmem es;
     const int nthr = NAT > 0 ? GT : (int)blockDim.x, nw = nthr >> 5;  // (the generic evaluator picks its CTA size at launch)
-    eval_smem_layout(ge, f.nblk, d.L, d.nb, d.nat, ga.nu, nw, NAT == 0, MIX, &es, smem_raw);
+    static_assert(!MG || (ORDER == 3 && !MIX), "global-memory Mhat: 3ph, FP64 only");
+    eval_smem_layout(ge, f.nblk, d.L, d.nb, d.nat, ga.nu, nw, NAT == 0, MIX, &es, smem_raw, MG);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nb = d.nb;
     const int NU = ga.nu;
     const int64_t gl = blockIdx.x / tiles_per_group;
@@ -513,7 +516,8 @@ __global__ void __launch_bounds__(NAT > 0 ? GT : GEN_WMAX * 32, NAT > 0 ? (MIX ?
             int t, lam1; int64_t rold;
             group_row<ORDER>(d, ga, G, rr0 + rt, t, lam1, rold);
             const double2 *src = pre + (size_t)t * nm9;
-            for (int i = threadIdx.x; i < nm9; i += nthr) es.M[rt * nm9 + i] = src[i];
+            if (!MG)
+                for (int i = threadIdx.x; i < nm9; i += nthr) es.M[rt * nm9 + i] = src[i];
         }
     } else {
         // level 1: Mhat_b[x][y] = sum_{c in b} phi(s1 q', Rj-Rl) sum_be T0[c][be][x][y] A'(j_c, be), A' = e~ (s1=+) or conj
@@ -587,7 +591,11 @@ __global__ void __launch_bounds__(NAT > 0 ? GT : GEN_WMAX * 32, NAT > 0 ? (MIX ?
         const unsigned *rp = es.rpre + rt * (NU + 1);
         const unsigned total = rp[NU];
         if (total == 0) continue;
-        bs.M = es.M + rt * nm9;
+        if (MG) {
+            int t, lam1; int64_t rold;
+            group_row<ORDER>(d, ga, G, rr0 + rt, t, lam1, rold);
+            bs.M = const_cast<double2 *>(pre) + (size_t)t * nm9;
+        } else bs.M = es.M + rt * nm9;
         const ListEnt *slot = lists + ((size_t)gl * ga.rmaxg + rr0 + rt) * NU * (size_t)capw;
         // the NU slots of the row read as one list: entry i lives in slot w = max{k : rp[k] <= i} at offset i - rp[w]
         auto fetch = [&](unsigned i) -> ListEnt {
@@ -694,35 +702,42 @@ cudaError_t launch_enum_g(int order, const FpDev &d, const GroupArgs &ga, int64_
 
 // warps of an evaluator CTA: 4, or -- generic atom count -- as many (at most GEN_WMAX) as the per-warp staging of 64
 // leg-A eigenvectors leaves room for beside the tile's tables
-static int eval_warps(const FpDev &d, const IfcDev &f, int ge) {
+static int eval_warps(const FpDev &d, const IfcDev &f, int ge, bool mglobal = false) {
     if (d.nat <= 2) return GW;
     int nw = GEN_WMAX;
-    while (nw > 1 && eval_smem_layout(ge, f.nblk, d.L, d.nb, d.nat, enum_units(d), nw, true, false, nullptr, nullptr) > 226 * 1024) nw--;
+    while (nw > 1 && eval_smem_layout(ge, f.nblk, d.L, d.nb, d.nat, enum_units(d), nw, true, false, nullptr, nullptr, mglobal) > 226 * 1024) nw--;
     return nw;
 }
-size_t eval_smem_bytes(const FpDev &d, const IfcDev &f, int ge) {              // (with the FP32 copies of the mixed mode)
-    return eval_smem_layout(ge, f.nblk, d.L, d.nb, d.nat, enum_units(d), eval_warps(d, f, ge), d.nat > 2, d.nat <= 2, nullptr, nullptr);
+size_t eval_smem_bytes(const FpDev &d, const IfcDev &f, int ge, bool mglobal) {   // (with the FP32 copies of the mixed mode)
+    return eval_smem_layout(ge, f.nblk, d.L, d.nb, d.nat, enum_units(d), eval_warps(d, f, ge, mglobal), d.nat > 2, d.nat <= 2 && !mglobal,
+                            nullptr, nullptr, mglobal);
 }
 
-template <int ORDER, int NAT, bool MIX>
+template <int ORDER, int NAT, bool MIX, bool MG = false>
 static cudaError_t launch_eval_t(const FpDev &d, const IfcDev &f, const GroupArgs &ga, int64_t ngc, const double2 *pre,
                                  int64_t capw, const ListEnt *lists, const uint32_t *wcnt, int ge, double2 *partial,
                                  uint32_t *counts, cudaStream_t st) {
-    const size_t smem = eval_smem_layout(ge, f.nblk, d.L, d.nb, d.nat, enum_units(d), eval_warps(d, f, ge), NAT == 0, MIX, nullptr, nullptr);
+    const int nw = eval_warps(d, f, ge, MG);
+    const size_t smem = eval_smem_layout(ge, f.nblk, d.L, d.nb, d.nat, enum_units(d), nw, NAT == 0, MIX, nullptr, nullptr, MG);
     const int tiles = (ga.rmaxg + ge - 1) / ge;
-    const unsigned nthr = 32u * (unsigned)eval_warps(d, f, ge);
+    const unsigned nthr = 32u * (unsigned)nw;
     static SmemGrant granted;
-    cudaError_t e = opt_in_smem(k_eval_g<ORDER, NAT, MIX>, smem, granted);
+    cudaError_t e = opt_in_smem(k_eval_g<ORDER, NAT, MIX, MG>, smem, granted);
     if (e != cudaSuccess) return e;
-    k_eval_g<ORDER, NAT, MIX><<<(unsigned)(ngc * tiles), nthr, smem, st>>>(d, f, ga, pre, capw, lists, wcnt, ge, tiles, partial, counts);
+    k_eval_g<ORDER, NAT, MIX, MG><<<(unsigned)(ngc * tiles), nthr, smem, st>>>(d, f, ga, pre, capw, lists, wcnt, ge, tiles, partial, counts);
     return cudaGetLastError();
 }
 
 cudaError_t launch_eval_g(int order, const FpDev &d, const IfcDev &f, const GroupArgs &ga, int64_t ngc, const double2 *pre,
                           int64_t capw, const ListEnt *lists, const uint32_t *wcnt, int ge, double2 *partial,
-                          uint32_t *counts, bool mixed, cudaStream_t st) {
+                          uint32_t *counts, bool mixed, bool mglobal, cudaStream_t st) {
     if (ngc <= 0) return cudaSuccess;
 #define FP_ARGS d, f, ga, ngc, pre, capw, lists, wcnt, ge, partial, counts, st
+    if (order == 3 && mglobal) {                                      // (FP64 only: the mixed mode needs the shared-memory copy)
+        if (d.nat == 1) return launch_eval_t<3, 1, false, true>(FP_ARGS);
+        if (d.nat == 2) return launch_eval_t<3, 2, false, true>(FP_ARGS);
+        return launch_eval_t<3, 0, false, true>(FP_ARGS);
+    }
     if (order == 3) {
         if (d.nat == 1) return mixed ? launch_eval_t<3, 1, true>(FP_ARGS) : launch_eval_t<3, 1, false>(FP_ARGS);
         if (d.nat == 2) return mixed ? launch_eval_t<3, 2, true>(FP_ARGS) : launch_eval_t<3, 2, false>(FP_ARGS);

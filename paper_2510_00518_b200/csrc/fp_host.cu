@@ -610,7 +610,9 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
                     "its per-row table needs " + std::to_string(need) + " bytes of shared memory, more than the 226 KB of one SM "
                     "(limit about 1,400 blocks)");
     };
-    if (rates_smem_bytes(d, f) > 227 * 1024 - 1024) return too_many_blocks(rates_smem_bytes(d, f));
+    // ... except for IFC3, whose Mhat is the level-0 table itself: past the limit the 3ph kernels read it from global memory
+    const bool mg = ifc_mglobal(d, f, order);
+    if (rates_smem_bytes(d, f, mg) > 227 * 1024 - 1024) return too_many_blocks(rates_smem_bytes(d, f, mg));
 
     // ---- scratch budget: per-target arrays for a super-chunk of targets ------------------------------------------------
     const size_t scratch_all = ctx->ws_bytes - ctx->resident;
@@ -652,8 +654,9 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
     if (split) {
         const size_t rowbytes = (size_t)f.nblk * 9 * sizeof(double2);
         ge = (int)std::max<size_t>(1, std::min<size_t>((size_t)rbound, FP_EVAL_TILE_BYTES / rowbytes));
+        if (mg) ge = std::min(rbound, 6);                             // (no table in shared memory: the rows of one q-point)
         if (order == 4 && ge >= njcap) ge = ge / njcap * njcap;      // whole targets: their rows share the level-0 loads
-        if (eval_smem_bytes(d, f, ge) > 227 * 1024 - 1024) return too_many_blocks(eval_smem_bytes(d, f, ge));
+        if (eval_smem_bytes(d, f, ge, mg) > 227 * 1024 - 1024) return too_many_blocks(eval_smem_bytes(d, f, ge, mg));
     }
     const size_t scratch = split ? scratch_all - list_region - 4096 : scratch_all;
     const size_t pre_per_target = (order == 3 ? (size_t)f.nblk * 9 : (size_t)f.n * 27) * sizeof(double2);
@@ -690,6 +693,7 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
         ra.overflow = reinterpret_cast<unsigned int *>(stat + 1);
         ra.evaluated = ctx->profiling ? stat + 2 : nullptr;
         ra.sym = 0;
+        ra.mglobal = mg ? 1 : 0;
         const int use_sym = (split && ctx->use_sym && (order == 4 ? ctx->sym34 : ctx->sym23)) ? 1 : 0;
         CU(cudaMemsetAsync(stat, 0, 3 * sizeof(unsigned long long), st));
         { ProfScope p(ctx, CAT_PRE, st);
@@ -759,7 +763,7 @@ static int rates_driver(fp_ctx *ctx, int order, const int32_t *targets, int64_t 
                     CU(cudaStreamWaitEvent(st, ctx->ev_enum[b], 0));
                 }
                 { ProfScope p(ctx, CAT_RATES, st);
-                  CU(launch_eval_g(order, d, f, gc, n, pre, capw, lists[b], wcnt[b], ge_t, partial, cnt, ctx->precision == FP_PREC_MIXED, st)); }
+                  CU(launch_eval_g(order, d, f, gc, n, pre, capw, lists[b], wcnt[b], ge_t, partial, cnt, ctx->precision == FP_PREC_MIXED, mg, st)); }
                 if (overlap) CU(cudaEventRecord(ctx->ev_eval[b], st));
             }
             unsigned long long novf = 0;
@@ -859,6 +863,7 @@ static int list_driver(fp_ctx *ctx, int order, int32_t target, int32_t channel, 
     CU(cudaMemcpyAsync(d_t, &target, 4, cudaMemcpyHostToDevice, st));
     RowArgs ra; ra.targets = d_t; ra.row0 = 0; ra.qp_begin = qp; ra.nqp = 1; ra.prefiltered = nullptr; ra.overflow = nullptr;
     ra.evaluated = nullptr; ra.sym = 0;
+    ra.mglobal = ifc_mglobal(d, order == 3 ? ctx->i3 : ctx->i4, order) ? 1 : 0;
     launch_count(order, d, ra, nrows, cnt, st);
     launch_scan(cnt, nrows, offs, bsums, st);
     std::vector<int64_t> ho(nrows + 1);
@@ -880,7 +885,7 @@ static int list_driver(fp_ctx *ctx, int order, int32_t target, int32_t channel, 
     if (ncopy > 0) CU(cudaMemcpyAsync(out, dec, ncopy * w * 4, cudaMemcpyDeviceToHost, st));
     if (terms && *n > 0) {                                            // per-process terms: level 0 of the target, then k_terms
         const IfcDev &f = order == 3 ? ctx->i3 : ctx->i4;
-        if (rates_smem_bytes(d, f) > 227 * 1024 - 1024) return fail(ctx, FP_ENOMEM, "IFC block table exceeds the shared memory of one SM");
+        if (rates_smem_bytes(d, f, ra.mglobal != 0) > 227 * 1024 - 1024) return fail(ctx, FP_ENOMEM, "IFC block table exceeds the shared memory of one SM");
         double2 *pre = sc.take<double2>(order == 3 ? (size_t)f.nblk * 9 : (size_t)f.n * 27);
         double *gp = sc.take<double>(*n);
         if (!pre || !gp) return fail(ctx, FP_ENOMEM, "scratch");

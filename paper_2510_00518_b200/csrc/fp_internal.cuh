@@ -76,6 +76,8 @@ struct RowArgs {
                                   // unordered pair of them once
     unsigned int *overflow;       // split path: += 1 for every (row, warp) list slot that filled up (the driver then
                                   // re-runs those rows through the fused kernel)
+    int mglobal;                  // 3ph only: the block table Mhat of a row is read from the level-0 table in global memory
+                                  // instead of a shared-memory copy (IFC3 lists too long for shared memory, ifc_mglobal())
 };
 
 // Group path: the targets of a super-chunk that share their q-point form a group; the rows of a group CTA -- 3ph:
@@ -142,7 +144,10 @@ void launch_pre4(const FpDev &d, const IfcDev &f, const int32_t *targets, int64_
 // only_flagged: redo pass of the split path -- only rows with counts[r] == 0xffffffff (a list slot filled up) are computed
 cudaError_t launch_rates(int order, const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const double2 *pre,
                          double2 *partial, uint32_t *counts, bool only_flagged, cudaStream_t st);
-size_t rates_smem_bytes(const FpDev &d, const IfcDev &f);
+size_t rates_smem_bytes(const FpDev &d, const IfcDev &f, bool mglobal = false);
+// true if the per-row table of an IFC3 list does not fit the shared memory of one SM: the 3ph kernels then read Mhat from
+// global memory (L1/L2) -- slower per block, but the list length is no longer capped by it (include/fourphonon.h, Limits)
+bool ifc_mglobal(const FpDev &d, const IfcDev &f, int order);
 // per-process terms of explicit lists (fp_terms3 / fp_terms4): row r of the launch is ra.row0 + blockIdx.x
 cudaError_t launch_terms(int order, const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const double2 *pre,
                          const int64_t *offsets, int64_t list_base, const uint32_t *list, double scale, double *gamma_p,
@@ -151,7 +156,7 @@ cudaError_t launch_terms(int order, const FpDev &d, const IfcDev &f, const RowAr
 #define FP_GROUP_RMAX 64          // rows of one enumerator group (they share the scan of the two free legs)
 int64_t enum_slot_entries(const FpDev &d);        // entries of one (row, warp) list slot that can never overflow
 int enum_units(const FpDev &d);                   // enumeration units per group CTA = list slots per row
-size_t eval_smem_bytes(const FpDev &d, const IfcDev &f, int ge);   // dynamic shared memory of an evaluator tile of ge rows
+size_t eval_smem_bytes(const FpDev &d, const IfcDev &f, int ge, bool mglobal = false);   // dynamic shared memory of an evaluator tile of ge rows
 // wcnt[(group CTA * rmaxg + row-in-group) * units + unit] = list entries written (0xffffffff: the slot filled up);
 // work: a device counter the launcher zeroes (the units are dealt to the warps of a persistent grid)
 cudaError_t launch_enum_g(int order, const FpDev &d, const GroupArgs &ga, int64_t ngc, int64_t capw, ListEnt *lists,
@@ -159,7 +164,7 @@ cudaError_t launch_enum_g(int order, const FpDev &d, const GroupArgs &ga, int64_
 // mixed: level-2 contraction in FP32 (nat <= 2 only; the generic evaluator stays FP64)
 cudaError_t launch_eval_g(int order, const FpDev &d, const IfcDev &f, const GroupArgs &ga, int64_t ngc, const double2 *pre,
                           int64_t capw, const ListEnt *lists, const uint32_t *wcnt, int ge, double2 *partial,
-                          uint32_t *counts, bool mixed, cudaStream_t st);
+                          uint32_t *counts, bool mixed, bool mglobal, cudaStream_t st);
 void launch_finalize(int order, const FpDev &d, int64_t nt, int64_t rows_per_unit, const double2 *partial,
                      const uint32_t *counts, double c_over_n, double *gamma, double *wp, int64_t *cnt, cudaStream_t st);
 void launch_kappa(const FpDev &d, const double *gamma_total, double pref, double *kappa, cudaStream_t st);

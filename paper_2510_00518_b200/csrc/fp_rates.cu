@@ -152,9 +152,10 @@ __device__ __forceinline__ bool row_is_empty(const FpDev &d, const Row &row) {
 template <int ORDER>
 __device__ __forceinline__ unsigned char *setup_row_tables(const FpDev &d, const IfcDev &f, const Row &row,
                                                            const double2 *pre, unsigned char *smem_raw, BlkSmem &bs,
-                                                           RowWeights &rw) {
-    bs.M = reinterpret_cast<double2 *>(smem_raw);
-    bs.ph = bs.M + 9 * f.nblk;
+                                                           RowWeights &rw, bool mglobal) {
+    const bool mg = ORDER == 3 && mglobal;                            // Mhat stays in the level-0 table (global memory)
+    bs.M = mg ? const_cast<double2 *>(pre) + (size_t)row.t * f.nblk * 9 : reinterpret_cast<double2 *>(smem_raw);
+    bs.ph = reinterpret_cast<double2 *>(smem_raw) + (mg ? 0 : 9 * f.nblk);
     double2 *e1 = bs.ph + d.L;                                        // nb entries (level 1 of ORDER 4)
     bs.meta = reinterpret_cast<int4 *>(e1 + d.nb);
     bs.seg = reinterpret_cast<int *>(bs.meta + f.nblk);
@@ -162,7 +163,8 @@ __device__ __forceinline__ unsigned char *setup_row_tables(const FpDev &d, const
     for (int i = threadIdx.x; i <= d.nat * d.nat; i += blockDim.x) bs.seg[i] = f.seg[i];
     if (ORDER == 3) {
         const double2 *src = pre + (size_t)row.t * f.nblk * 9;
-        for (int i = threadIdx.x; i < f.nblk * 9; i += blockDim.x) bs.M[i] = src[i];
+        if (!mg)
+            for (int i = threadIdx.x; i < f.nblk * 9; i += blockDim.x) bs.M[i] = src[i];
     } else {
         // level 1: Mhat_b[x][y] = sum_{c in b} phi(s1 q', Rj-Rl) sum_be T0[c][be][x][y] A'(j_c, be)
         for (int i = threadIdx.x; i < d.L; i += blockDim.x) {
@@ -308,7 +310,7 @@ __global__ void __launch_bounds__(RT, RATES_MINB) k_rates(FpDev d, IfcDev f, Row
     }
     BlkSmem bs;
     RowWeights rw;
-    uint2 *evq = reinterpret_cast<uint2 *>(setup_row_tables<ORDER>(d, f, row, pre, smem_raw, bs, rw));   // RW*QCAP
+    uint2 *evq = reinterpret_cast<uint2 *>(setup_row_tables<ORDER>(d, f, row, pre, smem_raw, bs, rw, ra.mglobal != 0));   // RW*QCAP
     uint2 *tailbuf = evq + RW * QCAP;                                                  // RW*32 (merged tails)
     uint32_t *pendq = reinterpret_cast<uint32_t *>(tailbuf + RW * 32);                // RW*PCAP
 
@@ -409,7 +411,7 @@ __global__ void __launch_bounds__(RT) k_terms(FpDev d, IfcDev f, RowArgs ra, con
     const Row row = make_row<ORDER>(d, ra, r);
     BlkSmem bs;
     RowWeights rw;
-    setup_row_tables<ORDER>(d, f, row, pre, smem_raw, bs, rw);
+    setup_row_tables<ORDER>(d, f, row, pre, smem_raw, bs, rw, ra.mglobal != 0);
     for (int64_t i0 = 0; i0 < cnt; i0 += RT) {
         const int64_t i = i0 + threadIdx.x;
         const bool act = i < cnt;
@@ -432,15 +434,15 @@ void launch_pre4(const FpDev &d, const IfcDev &f, const int32_t *targets, int64_
     if (nt > 0) k_pre4<<<(unsigned)nt, 256, 0, st>>>(d, f, targets, t0);
 }
 
-static size_t tables_smem_bytes(const FpDev &d, const IfcDev &f) {
-    return (size_t)f.nblk * 9 * sizeof(double2) + (size_t)d.L * sizeof(double2) + (size_t)d.nb * sizeof(double2) +
+static size_t tables_smem_bytes(const FpDev &d, const IfcDev &f, bool mglobal) {
+    return (mglobal ? 0 : (size_t)f.nblk * 9 * sizeof(double2)) + (size_t)d.L * sizeof(double2) + (size_t)d.nb * sizeof(double2) +
            (size_t)f.nblk * sizeof(int4) + (size_t)((d.nat * d.nat + 1 + 3) & ~3) * sizeof(int);
 }
 cudaError_t launch_terms(int order, const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const double2 *pre,
                          const int64_t *offsets, int64_t list_base, const uint32_t *list, double scale, double *gamma_p,
                          cudaStream_t st) {
     if (nrows <= 0) return cudaSuccess;
-    const size_t smem = (tables_smem_bytes(d, f) + 15) & ~(size_t)15;
+    const size_t smem = (tables_smem_bytes(d, f, ra.mglobal != 0) + 15) & ~(size_t)15;
     static SmemGrant g3, g4;
     if (order == 3) {
         cudaError_t e = opt_in_smem(k_terms<3>, smem, g3);
@@ -453,15 +455,16 @@ cudaError_t launch_terms(int order, const FpDev &d, const IfcDev &f, const RowAr
     }
     return cudaGetLastError();
 }
-size_t rates_smem_bytes(const FpDev &d, const IfcDev &f) {
-    size_t b = tables_smem_bytes(d, f) + (size_t)(RW * QCAP + RW * 32) * sizeof(uint2) + (size_t)(RW * PCAP) * sizeof(uint32_t);
+bool ifc_mglobal(const FpDev &d, const IfcDev &f, int order) { return order == 3 && rates_smem_bytes(d, f, false) > 226 * 1024; }
+size_t rates_smem_bytes(const FpDev &d, const IfcDev &f, bool mglobal) {
+    size_t b = tables_smem_bytes(d, f, mglobal) + (size_t)(RW * QCAP + RW * 32) * sizeof(uint2) + (size_t)(RW * PCAP) * sizeof(uint32_t);
     return (b + 15) & ~(size_t)15;
 }
 
 template <int ORDER, int NAT, int TILE>
 static cudaError_t launch_rates_t(const FpDev &d, const IfcDev &f, const RowArgs &ra, int64_t nrows, const double2 *pre,
                                   double2 *partial, uint32_t *counts, bool only_flagged, cudaStream_t st) {
-    const size_t smem = rates_smem_bytes(d, f);
+    const size_t smem = rates_smem_bytes(d, f, ra.mglobal != 0);
     static SmemGrant granted;
     cudaError_t e = opt_in_smem(k_rates<ORDER, NAT, TILE>, smem, granted);
     if (e != cudaSuccess) return e;

@@ -543,3 +543,37 @@ def test_mixed_precision_mode(fp):
         assert err.max() < 2e-5, (what, err.max())
     assert np.abs(g - g64).max() > 0.0
     assert_rates_close(g64, og, "Gamma4 (FP64)")
+
+
+def test_long_ifc3_list_reads_the_block_table_from_global_memory(fp):
+    """ADVICE.md / include/fourphonon.h "Limits": an IFC3 list with more contraction blocks (atomA, atomB, R_A - R_B mod mesh)
+    than the shared memory of one SM can hold as a per-row table (about 1,400) is still served -- the 3ph kernels then read
+    Mhat from the level-0 table in global memory.  A synthetic list of 1,700 triplets, one block each, on an 8x8x8 mesh: rates,
+    weighted phase space and counts of a few targets against the oracle on the group path and the fused path, and the
+    per-process terms."""
+    import copy
+    base = fp_inputs.make_tiny("diamond", mesh=(8, 8, 8), with4=False)
+    rng = np.random.default_rng(11)
+    n = 1700
+    combos = rng.permutation(4 * 512)[:n]                            # distinct (atom j, atom k, R_j - R_k mod 8)
+    aj, ak, dr = combos // 1024, (combos // 512) % 2, combos % 512
+    d3 = np.stack([dr % 8, (dr // 8) % 8, dr // 64], axis=1)
+    Rk = rng.integers(-1, 2, size=(n, 3))
+    atoms = np.stack([rng.integers(0, 2, size=n), aj, ak], axis=1).astype(np.int32)
+    cells = np.concatenate([Rk + d3, Rk], axis=1).reshape(n, 2, 3).astype(np.int32)
+    phi = rng.normal(0.0, 0.5, size=(n, 27))
+    inp = copy.copy(base)
+    inp.ifc3 = (np.ascontiguousarray(atoms), np.ascontiguousarray(cells), np.ascontiguousarray(phi))
+    t = np.array([5, 700, 1501, 3070], dtype=np.int32)
+    og, ow, oc = _oracle(inp).rates3(t)
+    assert oc.sum() > 1000
+    for path in (fp.FP_PATH_AUTO, fp.FP_PATH_FUSED):
+        with fp.Context.from_inputs(inp, scratch_bytes=1 << 30) as ctx:
+            ctx.set_path(path)
+            g, w, c = ctx.rates3(t)
+            assert np.array_equal(c, oc)
+            assert_rates_close(g, og, f"Gamma3 (long IFC3 list, path {path})")
+            assert_rates_close(w, ow, f"WP3 (long IFC3 list, path {path})")
+            if path == fp.FP_PATH_FUSED:
+                pairs, gp = ctx.terms3(int(t[1]), 1)
+                assert len(gp) == int(oc[1, 1]) and abs(gp.sum() - og[1, 1]) <= 1e-9 * abs(og[1, 1])
